@@ -1,0 +1,188 @@
+/*
+ * ia.h -- C-ABI boundary of the B200-native batched ion+atom trajectory propagator
+ * (the data-parallel hot path of arXiv 2509.15117, Chowdhury & Perez-Rios).
+ *
+ * What the library computes (citations are /root/reference/PAPER.md lines and DESIGN.md readings):
+ *   For each of n independent trajectories it integrates Newton's equations of the Hamiltonian of
+ *   Eq. 1-2 -- a Paul-trapped ion and a neutral atom interacting through
+ *   V(r) = C8/r^8 - C4/r^4, C4 = alpha/2, C8 = C4^2/(4 De) (BASELINE.json north_star) --
+ *   for the twelve variables (r_i, r_a, v_i, v_a) in FP64 atomic units with the adaptive fourth/fifth
+ *   order embedded Runge-Kutta pair of refs [22,23] (Dormand-Prince 5(4) with
+ *   the ode45 controller, reading R5), from "head-on" initial conditions to
+ *   the termination test (R7/R8), and reduces every trajectory on the device to its
+ *   scattering observables: final ion kinetic energy, number of short-range
+ *   collisions ("bounces") and of r(t) turning points, dwell time, complex lifetime, final atom
+ *   velocity (-> outgoing direction, scattering angle, momentum transfer).
+ *
+ * All of it runs in hand-written sm_100a CUDA kernels.  There is NO CPU fallback: on a machine
+ * without a compute-capability-10.x device ia_create fails with IA_EDEVICE.
+ *
+ * Conventions
+ *   - "device" pointers are CUDA device pointers valid on the ctx's device; "host" pointers are
+ *     ordinary process memory.  Each argument says which it is.
+ *   - The library never allocates, frees or keeps caller memory.  A ctx owns only its own scratch
+ *     (work counter, host-call staging buffers).
+ *   - Every function returns IA_OK (0) or a negative ia_status; on failure nothing was launched.
+ *     A failed *trajectory* is not a call error: see ia_record.status.
+ *   - A ctx is not thread-safe.  Two ctxs may run concurrently on different streams.
+ */
+#ifndef IA_H
+#define IA_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ia_ctx ia_ctx; /* opaque, owned by the library */
+
+typedef enum {
+    IA_OK = 0,
+    IA_EINVAL = -1,  /* NULL / non-finite / out-of-range argument                          */
+    IA_ENOMEM = -2,  /* host or device allocation of ctx scratch failed                    */
+    IA_ECUDA = -3,   /* a CUDA runtime call failed; text in ia_last_error                  */
+    IA_EDEVICE = -4  /* no CUDA device, or the device is not compute capability 10.x       */
+} ia_status;
+
+/* Species: masses in unified atomic mass units, static dipole polarisability of the
+ * atom in atomic units.  C4 = alpha/2. */
+typedef struct {
+    double m_ion_u, m_atom_u, alpha_au;
+} ia_species;
+
+/* Paul trap (Eq. 2): Mathieu parameters a_k, q_k per Cartesian axis k = x,y,z of
+ * the ION's coordinates (trap centre = origin) and the rf angular frequency in atomic units.
+ * Force on the ion: -(a_k + 2 q_k cos(Omega_rf t + phase)) m_ion Omega_rf^2/4 * r_k. */
+typedef struct {
+    double a[3], q[3], omega_rf_au;
+} ia_trap;
+
+/* Integration controls (readings R4, R5, R6, R8).  Zero in a field selects the default. */
+typedef struct {
+    double rtol;        /* relative tolerance, in [1e-13, 1e-3]; default 1e-10                       */
+    double atol;        /* absolute tolerance (a.u., one scalar for all 12 components); default 1e-12 */
+    double t_max_rf;    /* time limit in rf periods; default 1e4                                      */
+    double h_max_rf;    /* step-size cap in rf periods, in (0, 0.25]; default 0.25                    */
+    double r_coll_a0;   /* a minimum of r(t) counts as a bounce if r < r_coll; default 500 a0         */
+    uint64_t max_steps; /* cap on attempted steps per trajectory; default 2^31                        */
+} ia_tol;
+
+/* Creates a context for one (species, trap, De, r0, tolerances) cell on CUDA device `cuda_device`.
+ * All pointers are host pointers; *out receives the handle.  De_K is the well depth in kelvin
+ * (C8 = C4^2/(4 De)), r0_a0 the radius of the start/exit sphere in Bohr radii. */
+int ia_create(ia_ctx **out, const ia_species *species, const ia_trap *trap, double De_K, double r0_a0,
+              const ia_tol *tol, int cuda_device);
+
+typedef enum {
+    IA_IC_EXPLICIT = 0, /* caller supplies y0[n][12] and phase[n]                                  */
+    IA_IC_GRID = 1,     /* cell-centred uniform (theta,phi) grid, head-on (R1)      */
+    IA_IC_PHILOX = 2    /* Philox4x32-10(seed; index, cell) directions / phases / energies (R2)     */
+} ia_ic_mode;
+
+/* Initial conditions of one launch.  Trajectory j of the launch (0 <= j < n) has global index
+ * first_index + j; its outputs go to slot j. */
+typedef struct {
+    int32_t mode;          /* ia_ic_mode                                                            */
+    int32_t domain;        /* GRID/PHILOX: 0 = one octant, 1 = full sphere            */
+    int32_t phase_mode;    /* GRID/PHILOX: 0 = fixed phase0, 1 = uniform in [0,2pi) from Philox      */
+    uint32_t n_theta, n_phi; /* GRID: theta_i = (i+1/2) span/n_theta, i = j / n_phi; phi likewise   */
+    uint64_t n;            /* number of trajectories in this launch                                 */
+    const double *y0;      /* EXPLICIT: [n][12] = r_i, r_a, v_i, v_a (a.u.); device for ia_run,
+                              host for ia_run_host                                                  */
+    const double *phase;   /* EXPLICIT: [n] rf phase at t = 0 (rad); same residency as y0           */
+    double phase0;         /* fixed rf phase (rad)                                                  */
+    double E_min_uK, E_max_uK; /* collision energy E/k_B in microkelvin; equal -> fixed, else
+                              log-uniform from Philox (BASELINE.json configs[4])                   */
+    uint64_t seed;         /* PHILOX key                                                            */
+    uint32_t cell;         /* PHILOX counter word 2 (BASELINE.json configs[2]: Philox(seed,cell,index)) */
+    uint64_t first_index;  /* global index of trajectory 0 (GRID: must be 0 <= first_index, the
+                              grid position is first_index + j)                                     */
+} ia_launch;
+
+/* Per-trajectory outcome, 64 bytes, little-endian (R6, R7, R10). */
+typedef struct {
+    double ke_ion;      /* 1/2 m_i |v_i|^2 at termination (E_h)                                     */
+    double t_dwell;     /* time from start to termination (a.u.)                                    */
+    double t_life;      /* t(last bounce) - t(first bounce) if n_coll >= 2, else 0 (a.u.)           */
+    double va_f[3];     /* atom velocity at termination (a.u.)                                      */
+    uint32_t n_coll;    /* short-range collisions: minima of r(t) with r < r_coll                   */
+    uint32_t n_tp;      /* all turning points of r(t) (sign changes of d.w at accepted steps)       */
+    uint32_t steps_acc; /* accepted RK steps                                                        */
+    uint16_t steps_rej; /* rejected RK steps, saturating at 65535                                   */
+    uint8_t status;     /* 0 escaped (|d| > r0 after closest approach), 1 t_max reached,
+                           2 step size underflow, 3 non-finite initial state, 4 max_steps          */
+    uint8_t n_loc;      /* exit-localisation iterations used (R7)                                   */
+} ia_record;
+
+#define IA_HIST_BINS 32
+/* Ensemble reduction of one launch (R16), 512 bytes.  The library
+ * ACCUMULATES into it: the caller zeroes it before the first launch it should cover. */
+typedef struct {
+    uint64_t n_done;            /* trajectories finished                                            */
+    uint64_t n_status[5];       /* by ia_record.status                                              */
+    uint64_t n_complex;         /* n_coll >= 2 (more than a single bounce)             */
+    uint64_t steps_acc, steps_rej; /* totals (exact, not saturated); rejected excludes localisation */
+    uint64_t steps_loc;         /* extra uncontrolled steps spent localising exits                  */
+    double sum_ke, sum_ke2;     /* sum of ke_ion and ke_ion^2 over status == 0 trajectories (R16)    */
+    uint64_t hist_ncoll[IA_HIST_BINS]; /* bin 0: n_coll = 0; bin b >= 1: 2^(b-1) <= n_coll < 2^b    */
+    uint64_t t_first_idle_ns;   /* %globaltimer when the first lane found the work counter empty    */
+    uint64_t t_start_ns, t_end_ns; /* min / max %globaltimer over the kernel's warps                */
+    uint64_t warn;              /* bit 0: 10|V(r0)| >= E_min (PAPER.md:28 asymptotic-start rule)     */
+    uint64_t reserved[16];
+} ia_summary;
+
+typedef struct {
+    ia_record *records;  /* [n] or NULL                                                            */
+    ia_summary *summary; /* one ia_summary or NULL                                                 */
+    double *ic_dump;     /* [n][14] = y0[12], phase, E (E_h) as generated, or NULL                 */
+} ia_outputs;
+
+/* Enqueues the propagation of one launch on `cuda_stream` (a cudaStream_t; NULL = legacy default
+ * stream) and returns without synchronising.  Every pointer inside `launch` and `outputs` is a
+ * DEVICE pointer; outputs are valid once the stream has been synchronised by the caller.
+ * n = 0 is valid and launches nothing. */
+int ia_run(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *outputs, void *cuda_stream);
+
+/* Same computation with HOST buffers: copies launch->y0/phase (EXPLICIT mode) to ctx-owned device
+ * staging, runs, copies records / summary / ic_dump back and synchronises.  The host summary is
+ * overwritten (not accumulated).  This is the end-to-end entry bench.py times. */
+int ia_run_host(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *host_outputs);
+
+/* Generator only (R1-R3): ic_dump is a DEVICE buffer [n][14]. */
+int ia_generate(ia_ctx *ctx, const ia_launch *launch, double *ic_dump, void *cuda_stream);
+
+/* Verification entry points (BASELINE.json north_star: "fixed-step mode built with fmad off").
+ * use_fma = 0 runs the translation unit compiled with -fmad=false, 1 the production arithmetic.
+ *
+ * ia_step_map: n independent single uncontrolled DP5(4) steps.  DEVICE arrays t_frac[n] (time folded
+ * into [0,T_rf), R9), phase[n], y[n][12], h[n] in; ynew[n][12] and err[n] (the ode45 error norm of the
+ * step, R5) out.  err may be NULL.
+ * ia_trace: nsteps uncontrolled steps of size h from y0[12] (HOST pointer) with rf phase `phase`;
+ * states is a DEVICE buffer [nsteps+1][13] = (t, y) rows, row 0 the start. */
+int ia_step_map(ia_ctx *ctx, uint64_t n, const double *t_frac, const double *phase, const double *y,
+                const double *h, double *ynew, double *err, int use_fma, void *cuda_stream);
+int ia_trace(ia_ctx *ctx, const double *y0_host, double phase, double h, uint32_t nsteps, double *states,
+             int use_fma, void *cuda_stream);
+
+/* Derived constants as the device sees them (host pointer, 16 doubles):
+ * m_i, m_a, C4, C8, De, r_e, Omega, T_rf, thr, h_max, h_min, t_max, r0, r_coll, rtol, atol. */
+int ia_get_derived(const ia_ctx *ctx, double *out16);
+
+/* Launch geometry of ia_run on this ctx (host pointers): resident warps per SM, SM count,
+ * registers per thread and local-memory (spill) bytes per thread of the persistent kernel. */
+int ia_get_kernel_info(const ia_ctx *ctx, int *warps_per_sm, int *n_sm, int *regs_per_thread,
+                       int *local_bytes_per_thread);
+
+/* FP64 FMA peak microbenchmark (the roofline denominator): runs independent DFMA chains on every SM
+ * of `cuda_device` for about `target_ms` and reports the sustained rate.  Host pointers.
+ * tflops = 2 * DFMA/s / 1e12; elapsed_ms = CUDA-event time of the timed launch. */
+int ia_fp64_peak(int cuda_device, double target_ms, double *tflops, double *elapsed_ms);
+
+int ia_destroy(ia_ctx *ctx);
+const char *ia_strerror(int code);
+const char *ia_last_error(const ia_ctx *ctx); /* "" if none; valid until the next call on ctx */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* IA_H */
