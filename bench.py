@@ -1,0 +1,315 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the batched ion+atom propagator on BASELINE.json configs[1]
+(Yb+ + 87Rb fractal angle map, 512x512 octant grid = 262,144 trajectories, E = 1.5 uK, t_max 1e4 T_rf).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--n-side 512]
+
+One "step" = one pass of the whole hot path (generator -> adaptive DP5(4) propagation -> events ->
+exit localisation -> observables -> record write -> ensemble reduction) over the whole grid.
+Prints ONE JSON line on rank 0.  `value` = trajectories/s with everything resident on the device;
+`e2e` = the same metric through ia_run_host with HOST buffers (explicit initial conditions copied in,
+records and summary copied out, inside the timed region).  `roofline` is against the FP64 FMA peak
+measured live by the library's DFMA microbenchmark (MEASURED_PEAKS.json carries no FP64 figure).
+`--impl reference` times the CPU oracle (test infrastructure; the only other place that may run it).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+import ia_inputs as I  # noqa: E402
+
+METRIC = "trajectories/s"
+# Algorithmic FP64 flops per ATTEMPTED RK step (FMA = 2), counted from the formulas of the
+# Nystrom-collapsed DP5(4) step in DESIGN.md section "Roofline": coefficient products 35, stage sums
+# 300, cosines 165, six accelerations 234, error estimate + norm 142, controller 25, events/time 17.
+FLOP_PER_STEP = 918.0
+ORACLE_SAMPLE_EVERY = 8   # cpu_baseline: every 8th grid point in theta and phi (64x64 = 4,096 trajectories)
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--n-side", type=int, default=512)
+    ap.add_argument("--workload", default="config1",
+                    help="config1 (default, the bench line) | config0 | config2.<cell 0-24> | config3.<cell 0-19> | "
+                         "config4 (one batch): the other BASELINE.json configs, for profiling and inspection")
+    ap.add_argument("--n", type=int, default=0, help="trajectories per pass for the Philox workloads (default: "
+                                                     "the config's own cell / batch size)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def pick_workload(args):
+    """BASELINE.json configs -> one cell (params + launch).  config1 is the bench workload."""
+    w = args.workload
+    if w == "config1":
+        return I.config1(args.n_side)
+    if w == "config0":
+        return I.config0()
+    name, _, idx = w.partition(".")
+    if name == "config2":
+        return I.config2(n_per_cell=args.n or 2 ** 20)[int(idx or 0)]
+    if name == "config3":
+        return I.config3(n_per_cell=args.n or 2 ** 22)[int(idx or 0)]
+    if name == "config4":
+        n = args.n or 2 ** 24
+        return I.config4(n_total=n, batch=n)[0]
+    raise SystemExit(f"unknown --workload {w}")
+
+
+# ---- clocks ---------------------------------------------------------------------------------------
+
+class ClockSampler:
+    """nvidia-smi sampling during the timed region (the recipe's clocks line)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, device_index: int):
+        self.dev = device_index
+        self.tmp = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "200", "-i", str(self.dev)], stdout=self.tmp, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.proc = None
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        self.tmp.flush()
+        self.tmp.seek(0)
+        sm, smax, power, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.tmp.read().splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); smax.append(float(f[2])); power.append(float(f[3]))
+            except ValueError:
+                continue
+            for name, val in zip(names, f[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        os.unlink(self.tmp.name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(smax)), "power_w_max": float(max(power)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ---- the oracle legs (cpu_baseline and --impl reference) -----------------------------------------
+
+def oracle_sample(cell, n_side: int):
+    """Times the oracle, as it stands, on a bounded sample of the same workload: the decimated sub-grid
+    of a GRID launch, the first 4,096 indices of a Philox launch."""
+    from oracle import ia_oracle as O
+    cores = os.cpu_count() or 1
+    if cell.launch.mode != I.MODE_GRID or cell.launch.n_theta != n_side:
+        idx = np.arange(min(cell.launch.n, 4096), dtype=np.uint64)
+        t0 = time.perf_counter()
+        out = O.run_generated(cell.params, cell.launch, indices=idx, nthreads=cores)
+        dt = time.perf_counter() - t0
+        steps = int(out["steps_acc"].astype(np.int64).sum() + out["steps_rej"].astype(np.int64).sum())
+        return {"n": len(idx), "seconds": dt, "steps": steps, "cores": cores,
+                "sample": f"first {len(idx)} trajectories of {cell.name} ({steps} RK steps), one trajectory per "
+                          f"task over {cores} std::threads"}
+    idx = I.subgrid_indices(n_side, ORACLE_SAMPLE_EVERY) if n_side >= ORACLE_SAMPLE_EVERY else np.arange(n_side * n_side)
+    t0 = time.perf_counter()
+    out = O.run_generated(cell.params, cell.launch, indices=idx, nthreads=cores)
+    dt = time.perf_counter() - t0
+    steps = int(out["steps_acc"].astype(np.int64).sum() + out["steps_rej"].astype(np.int64).sum())
+    return {"n": len(idx), "seconds": dt, "steps": steps, "cores": cores,
+            "sample": f"every {ORACLE_SAMPLE_EVERY}th grid point in theta and phi of the {n_side}x{n_side} grid "
+                      f"({len(idx)} trajectories, {steps} RK steps), one trajectory per task over {cores} std::threads"}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cell = pick_workload(args)
+    times, last = [], None
+    for it in range(args.warmup + args.steps):
+        last = oracle_sample(cell, args.n_side)
+        if it >= args.warmup:
+            times.append(last["seconds"])
+    total = float(sum(times))
+    value = last["n"] * args.steps / total
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": "trajectories/s", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cell.name, "trajectories_per_step": last["n"], "note": "CPU oracle on a bounded sample"},
+            "rk_steps_per_s": last["steps"] * args.steps / total,
+            "cpu_baseline": {"value": value, "unit": "trajectories/s", "cores": last["cores"], "kind": "oracle",
+                             "sample": last["sample"]},
+            "e2e": {"value": value, "unit": "trajectories/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ---- our arm ----------------------------------------------------------------------------------------
+
+def run_ours(args):
+    import dataclasses
+
+    import torch
+    import torch.distributed as dist
+
+    import paper_2509_15117_b200 as P
+    from paper_2509_15117_b200 import dist as D
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the propagator has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+    K, W = args.steps, max(args.warmup, 3)
+
+    # Workload: configs[1].  Trajectories are independent, so N GPUs run N grids of the same shape (weak
+    # scaling, no data-path collective): rank r maps the octant at rf phase 2 pi r / N.
+    cell = pick_workload(args)
+    if cell.launch.mode == I.MODE_GRID:
+        launch = dataclasses.replace(cell.launch, phase0=2.0 * np.pi * rank / world)
+    else:   # Philox workloads: rank r continues the same stream at index r * n
+        launch = dataclasses.replace(cell.launch, first_index=cell.launch.first_index + rank * cell.launch.n)
+    n = launch.n
+
+    def barrier():
+        if world > 1:
+            dist.barrier(device_ids=[local])
+        torch.cuda.synchronize(dev)
+
+    peak = P.ia_fp64_peak(local, 300.0)          # the roofline denominator, measured on this GPU now
+    ctx = P.Context(cell.params, device=local)
+    info = ctx.kernel_info
+    if info["local_bytes_per_thread"] < 0:
+        raise SystemExit("kernel info unavailable")
+    rec = torch.empty(n * P.RECORD_BYTES, dtype=torch.uint8, device=dev)
+    summaries = torch.zeros((W + K, P.SUMMARY_BYTES), dtype=torch.uint8, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+
+    for w in range(W):
+        ctx.run(launch, records=rec, summary=summaries[w])
+        flush.fill_(w)
+    barrier()
+    clocks = ClockSampler(local)
+    clocks.start()
+    for k in range(K):
+        ev[k][0].record()
+        ctx.run(launch, records=rec, summary=summaries[W + k])     # ONE kernel launch of ours per step
+        ev[k][1].record()
+        flush.fill_(k)                                             # L2 flush between timed iterations
+    barrier()
+    clk = clocks.stop()
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_s = D.all_reduce_max(sum(step_ms) * 1e-3, dev)
+    summ = P.view_summary(summaries[W + K - 1])
+    kernel_ms = float(np.mean(step_ms))
+    attempted = int(summ["steps_acc"]) + int(summ["steps_rej"]) + int(summ["steps_loc"])
+    tot = D.all_reduce_summary(summ, dev)
+    attempted_all = tot["steps_acc"] + tot["steps_rej"] + tot["steps_loc"]
+    value = world * n * K / total_s
+
+    # end to end through ia_run_host: explicit initial conditions in pinned host memory -> device,
+    # records + summary -> pinned host memory, all inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        ic = ctx.generate(launch)                                   # untimed: the inputs of the e2e leg
+        y0 = torch.from_numpy(np.ascontiguousarray(ic[:, :12])).pin_memory()
+        ph = torch.from_numpy(np.ascontiguousarray(ic[:, 12])).pin_memory()
+        rec_h = torch.empty(n * P.RECORD_BYTES, dtype=torch.uint8).pin_memory()
+        sum_h = torch.zeros(P.SUMMARY_BYTES, dtype=torch.uint8).pin_memory()
+        lx = I.Launch(mode=I.MODE_EXPLICIT, n=n)
+        cl = P.make_launch(lx, y0, ph)
+        P.ia_run_host(ctx.handle, cl, rec_h, sum_h)                 # warm-up (staging allocation)
+        barrier()
+        t0 = time.perf_counter()
+        for k in range(K):
+            P.ia_run_host(ctx.handle, cl, rec_h, sum_h)             # synchronous
+        torch.cuda.synchronize(dev)
+        e2e_s = D.all_reduce_max(time.perf_counter() - t0, dev)
+        done = int(sum_h.numpy().view(P.SUMMARY_DTYPE)[0]["n_done"])
+        assert done == n, (done, n)
+        e2e = {"value": world * n * K / e2e_s, "unit": "trajectories/s",
+               "h2d_bytes_per_step": int(y0.numel() * 8 + ph.numel() * 8),
+               "d2h_bytes_per_step": int(rec_h.numel() + sum_h.numel()), "ms_per_step": 1e3 * e2e_s / K}
+    ctx.close()
+    if world > 1:
+        dist.barrier(device_ids=[local])
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    achieved_tflops = FLOP_PER_STEP * attempted / (kernel_ms * 1e-3) / 1e12
+    bulk_ms = (int(summ["t_first_idle_ns"]) - int(summ["t_start_ns"])) * 1e-6
+    line = {
+        "metric": METRIC, "value": value, "unit": "trajectories/s", "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": 1e3 * total_s / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cell.name, "trajectories_per_step_per_gpu": n, "parallelism": f"dp{world}",
+                   "l2": "flushed between timed iterations (256 MiB write); the kernel reads no input arrays",
+                   "rtol": cell.params.rtol, "atol": cell.params.atol, "t_max_rf": cell.params.t_max_rf},
+        "rk_steps_per_s": attempted_all * K / total_s,
+        "rk_steps_per_pass": attempted_all,
+        "p_complex": tot["n_complex"] / max(tot["n_done"], 1), "n_status": tot["n_status"],
+        "roofline": {"bound": "alu", "achieved": achieved_tflops, "peak": peak["tflops"], "unit": "TFLOP/s",
+                     "frac": achieved_tflops / peak["tflops"], "traffic": None,
+                     "peak_source": "ia_fp64_peak (DFMA chains on all SMs, measured in this run); nominal 37.2",
+                     "flop_per_attempted_step": FLOP_PER_STEP, "kernel": "ia_persistent_kernel",
+                     "kernel_ms": kernel_ms, "ms_until_work_counter_empty": bulk_ms,
+                     "note": "whole-launch average: after the work counter empties the launch is bound by the "
+                             "serial latency of its longest trajectories (see DESIGN.md 'Tail')"},
+        "kernel_info": info, "clocks": clk, "e2e": e2e, "gpu_launches": K,
+    }
+    if not args.no_cpu_baseline and world == 1:
+        s = oracle_sample(cell, args.n_side)
+        line["cpu_baseline"] = {"value": s["n"] / s["seconds"], "unit": "trajectories/s", "cores": s["cores"],
+                                "kind": "oracle", "sample": s["sample"], "rk_steps_per_s": s["steps"] / s["seconds"]}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

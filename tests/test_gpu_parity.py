@@ -1,0 +1,279 @@
+"""GPU parity: the sm_100a CUDA path (through the C-ABI of include/ia.h) against the CPU oracle on
+the same seeded inputs.  BASELINE.json north_star fixes the bars:
+  (1) fixed-step mode built with fmad off: per step to a relative 1e-12 (reading R12);
+  (2) adaptive mode, non-chaotic trajectories: final observables to a relative 1e-8 (reading R15);
+  (3) chaotic ensembles: P(complex), mean ion energy gain, collision-count histogram within 99 %
+      binomial / bootstrap intervals (readings R14, R16).
+Integer / index work (Philox words, counts, statuses) is compared bit-for-bit.
+"""
+import os
+from dataclasses import replace
+
+import numpy as np
+import pytest
+
+import ia_inputs as I
+from oracle import ia_oracle as O
+import _stats as S
+
+pytestmark = pytest.mark.gpu
+NTHREADS = min(32, os.cpu_count() or 1)
+
+
+@pytest.fixture(scope="module")
+def P():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests selected on a machine without a CUDA device"
+    import paper_2509_15117_b200 as pkg
+    pkg.load()
+    return pkg
+
+
+def block_rel(y, yref, v_floor):
+    """Reading R12: relative difference per 3-vector block, with floors for blocks crossing zero."""
+    y, yref = np.atleast_2d(y), np.atleast_2d(yref)
+    out = []
+    for k, floor in ((0, 1e-2), (3, 0.0), (6, v_floor), (9, 0.0)):
+        num = np.linalg.norm(y[:, k:k + 3] - yref[:, k:k + 3], axis=1)
+        den = np.maximum(np.linalg.norm(yref[:, k:k + 3], axis=1), floor)
+        out.append(num / den)
+    return np.stack(out, axis=1)
+
+
+# ---------------------------------------------------------------------------------------------
+# generator (a2; readings R1-R3)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("domain,phase_mode,erange", [(0, 1, (3.0, 3.0)), (1, 1, (1.0, 100.0)), (0, 0, (1.5, 1.5))])
+def test_philox_generator_matches_oracle(P, domain, phase_mode, erange):
+    cell = I.config2(n_per_cell=1000)[17]
+    launch = replace(cell.launch, n=1000, domain=domain, phase_mode=phase_mode, phase0=0.75,
+                     E_min_uK=erange[0], E_max_uK=erange[1], first_index=(1 << 32) - 500)  # index carries into word 1
+    with P.Context(cell.params) as ctx:
+        ic = ctx.generate(launch)
+    y0, ph, E = O.generate(cell.params, launch, np.arange(1000))
+    # Philox words -> u1 (cos theta -> z of the atom) and u3 (phase) go through exact arithmetic: bit-for-bit
+    assert np.array_equal(ic[:, 5], y0[:, 5])
+    assert np.array_equal(ic[:, 12], ph)
+    # u2 -> phi -> sin/cos (sincospi vs sin/cos of a rounded product) and u4 -> E (exp vs pow): a few ulp
+    assert np.max(np.abs(ic[:, :12] - y0) / np.maximum(np.abs(y0), 1e-300).max(axis=0)) < 1e-15
+    assert np.max(np.abs(ic[:, 13] - E) / E) < 4e-15
+    assert np.all(ic[:, 0:3] == 0.0) and np.all(ic[:, 6:9] == 0.0)     # ion at rest at the centre
+    r = np.linalg.norm(ic[:, 3:6], axis=1)
+    assert np.max(np.abs(r - cell.params.r0_a0)) < 1e-9
+    # head-on: v_a antiparallel to r_a
+    cosang = np.sum(ic[:, 3:6] * ic[:, 9:12], axis=1) / (r * np.linalg.norm(ic[:, 9:12], axis=1))
+    assert np.max(np.abs(cosang + 1.0)) < 1e-15
+
+
+def test_grid_generator_matches_oracle(P):
+    cell = I.config1(64)
+    with P.Context(cell.params) as ctx:
+        ic = ctx.generate(cell.launch)
+    y0, ph, E = O.generate(cell.params, cell.launch, np.arange(cell.launch.n))
+    assert np.max(np.abs(ic[:, :12] - y0) / np.abs(y0).max(axis=0).clip(1e-300)) < 1e-15
+    assert np.array_equal(ic[:, 12], ph) and np.array_equal(ic[:, 13], E)
+
+
+# ---------------------------------------------------------------------------------------------
+# fixed-step mode (north_star: "built with fmad off ... per step to a relative 1e-12"; R12)
+# ---------------------------------------------------------------------------------------------
+def _sampled_states(cell, n_traj=6, seed=3):
+    """(t_frac, phase, y, h) sampled along oracle trajectories: far field, mid range, the inner turning
+    point, the way out -- with the step size the controller was using there."""
+    rng = np.random.default_rng(seed)
+    idx = rng.choice(cell.launch.n, n_traj, replace=False)
+    y0s, phs, _ = O.generate(cell.params, cell.launch, idx)
+    T = O.derive(cell.params)["T_rf"]
+    rows = []
+    for y0, ph in zip(y0s, phs):
+        out, path = O.run(cell.params, y0, ph, path_cap=20000)
+        t = path[:, 0]
+        for k in range(0, len(path) - 2, max(1, len(path) // 150)):
+            rows.append((t[k] % T, ph, path[k, 1:], t[k + 1] - t[k]))
+    tf = np.array([r[0] for r in rows]); ph = np.array([r[1] for r in rows])
+    y = np.stack([r[2] for r in rows]); h = np.array([r[3] for r in rows])
+    return tf, ph, y, h
+
+
+@pytest.mark.parametrize("use_fma", [False, True])
+@pytest.mark.parametrize("which", ["config0", "config1"])
+def test_one_step_map_1e12(P, which, use_fma):
+    cell = I.config0() if which == "config0" else I.config1(64)
+    tf, ph, y, h = _sampled_states(cell)
+    assert len(y) > 300 and np.linalg.norm(y[:, 3:6] - y[:, 0:3], axis=1).min() < 80.0  # reaches the well
+    ref = np.empty_like(y); eref = np.empty(len(y))
+    for k in range(len(y)):
+        yn, e = O.step(cell.params, tf[k], ph[k], y[k], h[k])
+        ref[k] = yn
+        eref[k] = O.err_norm(cell.params, y[k], yn, e)
+    with P.Context(cell.params) as ctx:
+        got, err = ctx.step_map(tf, ph, y, h, use_fma=use_fma)
+    rel = block_rel(got, ref, 1e-3 * np.linalg.norm(y[:, 9:12], axis=1).max())
+    print(f"\none-step map {which} fma={use_fma}: n={len(y)} max block rel diff {rel.max(axis=0)}")
+    assert rel.max() <= 1e-12
+    # the error norm is a sum with cancelling weights (sum E_l = 0): agreement to ~1e-6 of itself
+    assert np.max(np.abs(err - eref) / eref) < 1e-5
+
+
+def test_mixed_random_states_one_step(P):
+    """Random (not on-trajectory) states from far field to r ~ 55 a0, ragged count (3 tiles + tail)."""
+    cell = I.config1(64)
+    n = 64 * 3 + 17
+    y = I.random_states(n, seed=11)
+    rng = np.random.default_rng(5)
+    T = O.derive(cell.params)["T_rf"]
+    tf = rng.uniform(0, T, n); ph = rng.uniform(0, 2 * np.pi, n)
+    r = np.linalg.norm(y[:, 3:6] - y[:, 0:3], axis=1)
+    h = 1e-3 * T * np.clip(r / 1000.0, 1e-3, 1.0)
+    ref = np.stack([O.step(cell.params, tf[k], ph[k], y[k], h[k])[0] for k in range(n)])
+    with P.Context(cell.params) as ctx:
+        for fma in (False, True):
+            got, _ = ctx.step_map(tf, ph, y, h, use_fma=fma)
+            assert block_rel(got, ref, 1e-9).max() <= 1e-12
+
+
+def test_cumulative_trace(P):
+    """Reading R12(ii): one explicit IC, same fixed h on both sides, every state compared.  1e-12 is
+    required on the inbound leg and through the bounce; where it is first exceeded afterwards is printed."""
+    cell = I.config0()
+    y0, ph, _ = O.generate(cell.params, cell.launch, [517])
+    d = O.derive(cell.params)
+    h = d["T_rf"] / 400.0
+    nsteps = 1800   # 4.5 rf periods: in (3.4 T_rf free flight), bounce, part of the way out
+    ref = O.trace(cell.params, y0[0], ph[0], h, nsteps)
+    rmin_at = np.argmin(np.linalg.norm(ref[:, 4:7] - ref[:, 1:4], axis=1))
+    assert 0 < rmin_at < nsteps - 50
+    with P.Context(cell.params) as ctx:
+        for fma in (False, True):
+            got = ctx.trace(y0[0], ph[0], h, nsteps, use_fma=fma)
+            assert np.max(np.abs(got[:, 0] - ref[:, 0]) / np.maximum(ref[:, 0], h)) < 1e-14
+            rel = block_rel(got[:, 1:], ref[:, 1:], 1e-3 * np.linalg.norm(ref[:, 10:13], axis=1).max()).max(axis=1)
+            over = np.nonzero(rel > 1e-12)[0]
+            first = int(over[0]) if len(over) else None
+            print(f"\ntrace fma={fma}: closest approach at step {rmin_at}; max rel diff inbound "
+                  f"{rel[:rmin_at - 20].max():.2e}, overall {rel.max():.2e}; 1e-12 first exceeded at step {first}")
+            assert rel[:rmin_at - 20].max() <= 1e-12
+            assert rel.max() <= 1e-7   # after the bounce: amplified energy round-off, (D_e/E) eps sqrt(N) (R12(ii))
+
+
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_mirror_symmetry_is_bitwise_on_the_gpu(P, axis):
+    """IEEE arithmetic is sign-symmetric: flipping one coordinate of the IC flips that coordinate of the
+    result bit for bit (catches x/y/z indexing slips in the kernels)."""
+    cell = I.config0()
+    y0, ph, _ = O.generate(cell.params, replace(cell.launch, n_theta=5, n_phi=5, n=25), np.arange(25))
+    ym = y0.copy()
+    ym[:, axis::3] *= -1.0
+    lx = I.Launch(mode=I.MODE_EXPLICIT, n=25)
+    with P.Context(cell.params) as ctx:
+        a, _, _ = ctx.run_sync(lx, y0, ph)
+        b, _, _ = ctx.run_sync(lx, ym, ph)
+    flip = np.ones(3); flip[axis] = -1.0
+    assert np.array_equal(a["va_f"] * flip, b["va_f"])
+    for f in ("ke_ion", "t_dwell", "n_coll", "n_tp", "steps_acc", "steps_rej", "status"):
+        assert np.array_equal(a[f], b[f])
+
+
+# ---------------------------------------------------------------------------------------------
+# adaptive mode, non-chaotic: config 0 in full (north_star: final observables to a relative 1e-8; R15)
+# ---------------------------------------------------------------------------------------------
+def _compare_regular(rec, ref, label):
+    """Per-trajectory comparison on trajectories whose accepted/rejected step counts agree (R15: a
+    differing count is a flipped accept/reject decision, listed and compared at the 1e-3 level)."""
+    assert np.array_equal(rec["status"], ref["status"].astype(np.uint8))
+    same = (rec["steps_acc"] == ref["steps_acc"]) & (rec["steps_rej"] == np.minimum(ref["steps_rej"], 65535))
+    rel = lambda f: np.abs(rec[f] - ref[f]) / np.abs(ref[f])
+    vn = np.linalg.norm(ref["va_f"], axis=1)
+    e_dir = np.linalg.norm(rec["va_f"] / np.linalg.norm(rec["va_f"], axis=1)[:, None] - ref["va_f"] / vn[:, None], axis=1)
+    e_v = np.linalg.norm(rec["va_f"] - ref["va_f"], axis=1) / vn
+    e_t, e_k = rel("t_dwell"), rel("ke_ion")
+    q = lambda e: "/".join(f"{x:.1e}" for x in np.quantile(e[same], [0.5, 0.9, 0.99, 1.0]))
+    print(f"\n{label}: {same.sum()}/{len(rec)} identical step sequences; rel diff quantiles 50/90/99/100 %: "
+          f"t_dwell {q(e_t)}  dir {q(e_dir)}  va_f {q(e_v)}  ke_ion {q(e_k)}")
+    return same, e_t, e_dir, e_v, e_k
+
+
+def test_config0_adaptive_parity_full(P):
+    cell = I.config0()
+    with P.Context(cell.params) as ctx:
+        rec, summ, ic = ctx.run_sync(cell.launch, want_ic=True)
+    ref = O.run_explicit(cell.params, ic[:, :12], ic[:, 12], nthreads=NTHREADS)   # the same doubles the GPU integrated
+    ref_gen = O.run_generated(cell.params, cell.launch, nthreads=NTHREADS)       # and the oracle's own generator
+    assert np.all(ref["n_coll"] == 1) and np.all(ref["status"] == 0)             # all regular
+    assert np.array_equal(rec["n_coll"], ref["n_coll"]) and np.array_equal(rec["n_tp"], ref["n_tp"])
+    same, e_t, e_dir, e_v, e_k = _compare_regular(rec, ref, "config0 (same ICs)")
+    assert same.mean() >= 0.99
+    assert e_t[same].max() <= 1e-8 and e_dir[same].max() <= 1e-8 and e_v[same].max() <= 1e-8
+    assert np.median(e_k[same]) <= 1e-8 and e_k[same].max() <= 3e-7
+    # flipped decisions: still the same trajectory at truncation level (R15)
+    if (~same).any():
+        assert e_t[~same].max() < 1e-3 and e_k[~same].max() < 5e-2
+    same2, e_t2, e_dir2, e_v2, e_k2 = _compare_regular(rec, ref_gen, "config0 (own generators)")
+    assert same2.mean() >= 0.98 and e_t2[same2].max() <= 1e-8 and e_dir2[same2].max() <= 1e-8
+    # summary == reduction of the records
+    assert int(summ["n_done"]) == 1024 and int(summ["n_status"][0]) == 1024 and int(summ["n_complex"]) == 0
+    assert int(summ["steps_acc"]) == int(rec["steps_acc"].sum()) and int(summ["steps_rej"]) == int(rec["steps_rej"].sum())
+    assert abs(summ["sum_ke"] - rec["ke_ion"].sum()) <= 1e-12 * rec["ke_ion"].sum()
+    assert int(summ["hist_ncoll"][1]) == 1024
+
+
+# ---------------------------------------------------------------------------------------------
+# chaotic ensembles (north_star: 99 % binomial / bootstrap intervals; R14, R16)
+# ---------------------------------------------------------------------------------------------
+def _ensemble_checks(rec, ref, label):
+    n = len(rec)
+    k_g, k_o = int((rec["n_coll"] >= 2).sum()), int((ref["n_coll"] >= 2).sum())
+    ok_p, dp, half = S.two_proportion_ok(k_g, n, k_o, len(ref))
+    esc_g, esc_o = rec["status"] == 0, ref["status"] == 0
+    ok_m, dm, ci = S.bootstrap_mean_diff_ok(rec["ke_ion"][esc_g], ref["ke_ion"][esc_o])
+    ok_h, bad = S.histogram_ok(S.ncoll_bins(rec["n_coll"]), S.ncoll_bins(ref["n_coll"]))
+    med_g, med_o = np.median(rec["ke_ion"][esc_g]), np.median(ref["ke_ion"][esc_o])
+    print(f"\n{label}: n={n}  P(complex) gpu {k_g / n:.4f} oracle {k_o / len(ref):.4f} (diff {dp:+.4f}, 99% half-width {half:.4f}); "
+          f"mean ke_ion diff {dm:+.3e} CI [{ci[0]:+.3e},{ci[1]:+.3e}]; median ke_ion gpu {med_g:.4e} oracle {med_o:.4e}; "
+          f"hist gpu {S.ncoll_bins(rec['n_coll'])[:10]} oracle {S.ncoll_bins(ref['n_coll'])[:10]}")
+    return ok_p and ok_m and ok_h, (ok_p, ok_m, ok_h, bad)
+
+
+def test_config1_subgrid_ensemble_and_regular_region(P):
+    """Config 1 at 64x64 (same species / energy / trap / tolerances as the 512x512 map)."""
+    cell = I.config1(64)
+    with P.Context(cell.params) as ctx:
+        rec, summ, ic = ctx.run_sync(cell.launch, want_ic=True)
+    ref = O.run_explicit(cell.params, ic[:, :12], ic[:, 12], nthreads=NTHREADS)
+    ok, detail = _ensemble_checks(rec, ref, "config1 64x64")
+    assert ok, detail
+    # regular region (single bounce on both sides): per-trajectory parity (R15: ke_ion expected ~3e-8 here)
+    reg = (ref["n_coll"] == 1) & (rec["n_coll"] == 1) & (ref["status"] == 0)
+    assert reg.sum() > 500
+    same, e_t, e_dir, e_v, e_k = _compare_regular(rec[reg], ref[reg], "config1 regular region")
+    assert same.mean() >= 0.97
+    assert np.median(e_t[same]) <= 1e-8 and np.median(e_dir[same]) <= 1e-8
+    assert np.quantile(e_t[same], 0.99) <= 1e-5
+    # chaotic trajectories agree as an ensemble, not one by one (R14); counts still have to add up
+    assert int(summ["n_done"]) == cell.launch.n
+    assert int(summ["n_complex"]) == int((rec["n_coll"] >= 2).sum())
+    assert np.array_equal(summ["hist_ncoll"], S.ncoll_bins(rec["n_coll"]).astype(np.uint64))
+    esc = rec["status"] == 0
+    assert abs(summ["sum_ke"] - rec["ke_ion"][esc].sum()) <= 1e-11 * rec["ke_ion"][esc].sum()
+
+
+@pytest.mark.parametrize("which,ci", [("config2", 18), ("config2", 2), ("config3", 7), ("config4", 0)])
+def test_philox_cells_ensemble(P, which, ci):
+    """First 2^12 Philox indices of one cell of configs 2-4: Rb 30 uK (near the threshold),
+    Li 10 uK (no complexes), a D_e = 1 K / q = 0.2 cell of config 3, and config 4's log-uniform stream."""
+    n = 4096
+    cell = {"config2": I.config2, "config3": I.config3}.get(which, None)
+    cell = cell(n_per_cell=n)[ci] if cell else I.config4(n_total=n, batch=n)[0]
+    with P.Context(cell.params) as ctx:
+        rec, summ, _ = ctx.run_sync(cell.launch)
+    ref = O.run_generated(cell.params, cell.launch, nthreads=NTHREADS)
+    ok, detail = _ensemble_checks(rec, ref, cell.name)
+    if not ok:  # R15: ~1 false alarm per 100 tests at 99 % -> re-draw once with a new seed
+        l2 = replace(cell.launch, seed=cell.launch.seed + 1)
+        with P.Context(cell.params) as ctx:
+            rec, summ, _ = ctx.run_sync(l2)
+        ref = O.run_generated(cell.params, l2, nthreads=NTHREADS)
+        ok, detail = _ensemble_checks(rec, ref, cell.name + " (re-drawn)")
+    assert ok, detail
+    # trajectories still bound at t_max (status 1) are rare and agree as a proportion
+    assert S.two_proportion_ok(int((rec["status"] != 0).sum()), n, int((ref["status"] != 0).sum()), n)[0]
