@@ -1,0 +1,168 @@
+"""Host-side logic that needs no GPU: the Nystrom-collapsed tableau constants the kernels carry
+(re-derived here in exact rational arithmetic from the Dormand-Prince tableau of ref [22],
+PAPER.md:106), the input recipes of BASELINE.json's configs, index sharding, and the multi-process
+summary reduction (gloo, world_size 2)."""
+import os
+import re
+import socket
+from fractions import Fraction as F
+
+import numpy as np
+import pytest
+
+import ia_inputs as I
+from paper_2509_15117_b200 import dist as D
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+# Dormand & Prince 1980, RK5(4)7M -- typed here from the published tableau (independent of oracle/ and csrc/)
+C_ = [F(0), F(1, 5), F(3, 10), F(4, 5), F(8, 9), F(1), F(1)]
+A_ = [[], [F(1, 5)], [F(3, 40), F(9, 40)], [F(44, 45), F(-56, 15), F(32, 9)],
+      [F(19372, 6561), F(-25360, 2187), F(64448, 6561), F(-212, 729)],
+      [F(9017, 3168), F(-355, 33), F(46732, 5247), F(49, 176), F(-5103, 18656)],
+      [F(35, 384), F(0), F(500, 1113), F(125, 192), F(-2187, 6784), F(11, 84)]]
+BH_ = [F(5179, 57600), F(0), F(7571, 16695), F(393, 640), F(-92097, 339200), F(187, 2100), F(1, 40)]
+
+
+def amat():
+    a = [[F(0)] * 7 for _ in range(7)]
+    for s, row in enumerate(A_):
+        for l, v in enumerate(row):
+            a[s][l] = v
+    return a
+
+
+def device_macros():
+    """IA_* rational constants of csrc/ia_dev.cuh as exact Fractions."""
+    text = open(os.path.join(ROOT, "paper_2509_15117_b200", "csrc", "ia_dev.cuh")).read()
+    out = {}
+    for name, num, den in re.findall(r"#define\s+(IA_[A-Z]+\d+)\s+\((-?\d+)\.0\s*/\s*(\d+)\.0\)", text):
+        out[name] = F(int(num), int(den))
+    return out
+
+
+def test_collapsed_tableau_constants_are_the_exact_products():
+    """abar = a.a, ebar = (b - bhat).a, E = b - bhat: the second-order form the kernels integrate is
+    algebraically the first-order DP5(4) step for dx/dt = v, dv/dt = A(t, x)."""
+    a = amat()
+    b = a[6]
+    m = device_macros()
+    assert len(m) == 34
+    abar = [[sum(a[s][j] * a[j][l] for j in range(7)) for l in range(7)] for s in range(7)]
+    E = [b[l] - BH_[l] for l in range(7)]
+    ebar = [sum(E[j] * a[j][l] for j in range(7)) for l in range(7)]
+    seen = set()
+    for s in range(2, 7):
+        for l in range(7):
+            key = f"IA_AB{s + 1}{l + 1}"
+            if abar[s][l] != 0:
+                assert m[key] == abar[s][l], key
+                seen.add(key)
+            else:
+                assert key not in m
+        assert sum(abar[s]) == C_[s] ** 2 / 2                  # row sums of a.a (order-2 condition per stage)
+    for l in range(7):
+        for pre, vec in (("IA_B", b), ("IA_E", E), ("IA_EB", ebar)):
+            key = f"{pre}{l + 1}"
+            if vec[l] != 0:
+                assert m[key] == vec[l], key
+                seen.add(key)
+            else:
+                assert key not in m, key
+    for s in range(1, 5):
+        assert m[f"IA_C{s + 1}"] == C_[s]
+    assert sum(E) == 0 and sum(ebar) == sum(E[j] * C_[j] for j in range(7))
+    assert seen | {f"IA_C{k}" for k in (2, 3, 4, 5)} == set(m)   # no stray constant
+
+
+def test_config_recipes_match_baseline_json():
+    import json
+    cfg = json.load(open(os.path.join(ROOT, "BASELINE.json")))["configs"]
+    c0, c1 = I.config0(), I.config1()
+    assert "32" in cfg[0] and c0.launch.n == 1024 and c0.params.t_max_rf == 2000 and c0.launch.E_min_uK == 10.0
+    assert c0.params.m_atom_u == 7.016 and c0.params.alpha_au == 164.1 and c0.params.m_ion_u == 173.94
+    assert c0.params.q == (0.1, -0.1, 0.0) and c0.params.a == (-0.0005, -0.0005, 0.001)
+    assert c0.params.rtol == 1e-10 and c0.params.atol == 1e-12 and c0.params.r0_a0 == 5000.0
+    assert abs(c0.params.omega_rf_au - 3.0396596921148e-10) < 1e-22
+    assert c1.launch.n == 262144 and c1.params.m_atom_u == 86.909 and c1.params.alpha_au == 319.2
+    assert c1.launch.E_min_uK == 1.5 and c1.params.t_max_rf == 1e4 and c1.launch.phase_mode == 0
+    c2 = I.config2()
+    assert len(c2) == 25 and all(c.launch.n == 2 ** 20 and c.launch.domain == 0 and c.launch.phase_mode == 1 for c in c2)
+    assert len({c.launch.cell for c in c2}) == 25 and len({c.launch.seed for c in c2}) == 1
+    assert sorted({c.params.alpha_au for c in c2}) == [162.7, 164.1, 290.0, 319.2, 401.0]
+    c3 = I.config3()
+    assert len(c3) == 20 and all(c.launch.n == 2 ** 22 and c.launch.E_min_uK == 3.0 for c in c3)
+    assert sorted({c.params.De_K for c in c3}) == [0.1, 1.0, 10.0, 100.0]
+    assert all(c.params.q[0] == -c.params.q[1] and c.params.q[2] == 0.0 for c in c3)
+    c4 = I.config4()
+    assert len(c4) == 18 and sum(c.launch.n for c in c4) == 300_000_000 and c4[-1].launch.n == 14_787_328
+    assert all(c.launch.domain == 1 and (c.launch.E_min_uK, c.launch.E_max_uK) == (1.0, 100.0) for c in c4)
+    firsts = [c.launch.first_index for c in c4]
+    assert firsts == [k * 2 ** 24 for k in range(18)]                        # one Philox stream, advancing
+
+
+def test_subgrid_and_shards_tile_the_index_range():
+    idx = I.subgrid_indices(512, 8)
+    assert len(idx) == 4096 and len(set(idx.tolist())) == 4096 and idx.max() < 512 * 512
+    for n, world in ((262144, 8), (1000, 7), (5, 8), (0, 3)):
+        spans = [D.shard_range(n, r, world) for r in range(world)]
+        assert spans[0][0] == 0 and sum(c for _, c in spans) == n
+        for (f0, c0), (f1, _) in zip(spans, spans[1:]):
+            assert f0 + c0 == f1
+        assert max(c for _, c in spans) - min(c for _, c in spans) <= 1
+    l = I.config4(n_total=1000, batch=1000)[0].launch
+    parts = [D.shard_launch(l, r, 3) for r in range(3)]
+    assert [p.first_index for p in parts] == [0, 334, 667] and [p.n for p in parts] == [334, 333, 333]
+    with pytest.raises(ValueError):
+        D.shard_range(10, 3, 3)
+
+
+def _summary(seed):
+    import paper_2509_15117_b200 as P
+    rng = np.random.default_rng(seed)
+    s = np.zeros(1, dtype=P.SUMMARY_DTYPE)[0]
+    s["n_done"] = rng.integers(1, 1 << 40)
+    s["n_status"] = rng.integers(0, 1 << 30, 5)
+    s["n_complex"] = rng.integers(0, 1 << 30)
+    s["steps_acc"], s["steps_rej"], s["steps_loc"] = rng.integers(0, 1 << 50, 3)
+    s["sum_ke"], s["sum_ke2"] = rng.random(2)
+    s["hist_ncoll"] = rng.integers(0, 1 << 30, 32)
+    return s
+
+
+def _gloo_worker(rank, world, port, q):
+    import torch.distributed as dist
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    tot = D.all_reduce_summary(_summary(100 + rank))
+    tmax = D.all_reduce_max(1.5 + rank)
+    first, count = D.shard_range(1001, rank, world)
+    dist.destroy_process_group()
+    q.put((rank, tot, tmax, first, count))
+
+
+def test_summary_reduction_over_two_gloo_ranks():
+    """N > 1 path (no data-path collective): index-range shards + one sum of the summaries + max of times."""
+    import torch.multiprocessing as mp
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_gloo_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted([q.get(timeout=120) for _ in procs], key=lambda r: r[0])
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    a, b = _summary(100), _summary(101)
+    for rank, tot, tmax, first, count in res:
+        assert tmax == 2.5
+        assert tot["n_done"] == int(a["n_done"]) + int(b["n_done"])
+        assert tot["n_status"] == [int(x) + int(y) for x, y in zip(a["n_status"], b["n_status"])]
+        assert tot["hist_ncoll"] == [int(x) + int(y) for x, y in zip(a["hist_ncoll"], b["hist_ncoll"])]
+        assert tot["steps_acc"] == int(a["steps_acc"]) + int(b["steps_acc"])
+        assert abs(tot["sum_ke"] - (a["sum_ke"] + b["sum_ke"])) < 1e-15
+    assert (res[0][3], res[0][4], res[1][3], res[1][4]) == (0, 501, 501, 500)
