@@ -50,6 +50,8 @@ def parse():
                          "config4 (one batch): the other BASELINE.json configs, for profiling and inspection")
     ap.add_argument("--n", type=int, default=0, help="trajectories per pass for the Philox workloads (default: "
                                                      "the config's own cell / batch size)")
+    ap.add_argument("--t-max-rf", type=float, default=0.0,
+                    help="override the time limit (rf periods) -- profiling runs only; the bench line uses the config's own")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -57,6 +59,15 @@ def parse():
 
 def pick_workload(args):
     """BASELINE.json configs -> one cell (params + launch).  config1 is the bench workload."""
+    cell = _pick_workload(args)
+    if args.t_max_rf > 0.0:
+        import dataclasses
+        cell = dataclasses.replace(cell, name=f"{cell.name}_tmax{args.t_max_rf:g}",
+                                   params=dataclasses.replace(cell.params, t_max_rf=args.t_max_rf))
+    return cell
+
+
+def _pick_workload(args):
     w = args.workload
     if w == "config1":
         return I.config1(args.n_side)
