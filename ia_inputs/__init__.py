@@ -70,6 +70,7 @@ class Launch:
     seed: int = 0
     cell: int = 0
     first_index: int = 0
+    path: int = 0              # 0 production kernel pair, 1 bulk kernel only, 2 cooperative kernel only
 
 
 @dataclass(frozen=True)

@@ -79,6 +79,17 @@ typedef enum {
     IA_IC_PHILOX = 2    /* Philox4x32-10(seed; index, cell) directions / phases / energies (R2)     */
 } ia_ic_mode;
 
+/* Which kernels propagate a launch.  The bulk kernel runs one lane per trajectory; once the work
+ * counter is empty and a warp is down to a few running lanes (ia_set_handoff) it hands them to the
+ * cooperative kernel (three lanes per trajectory, a third of the FP64 instructions per lane and
+ * step), which finishes the long stragglers at a lower latency per step.  Both run the same
+ * arithmetic and give bit-identical records. */
+typedef enum {
+    IA_PATH_AUTO = 0,      /* bulk kernel, stragglers handed to the cooperative kernel             */
+    IA_PATH_BULK_ONLY = 1, /* bulk kernel to the end                                                */
+    IA_PATH_COOP_ONLY = 2  /* cooperative kernel from the first step (verification)                */
+} ia_path;
+
 /* Initial conditions of one launch.  Trajectory j of the launch (0 <= j < n) has global index
  * first_index + j; its outputs go to slot j. */
 typedef struct {
@@ -86,6 +97,7 @@ typedef struct {
     int32_t domain;        /* GRID/PHILOX: 0 = one octant, 1 = full sphere            */
     int32_t phase_mode;    /* GRID/PHILOX: 0 = fixed phase0, 1 = uniform in [0,2pi) from Philox      */
     uint32_t n_theta, n_phi; /* GRID: theta_i = (i+1/2) span/n_theta, i = j / n_phi; phi likewise   */
+    int32_t path;          /* ia_path: which kernels propagate (0 = the production pair)            */
     uint64_t n;            /* number of trajectories in this launch                                 */
     const double *y0;      /* EXPLICIT: [n][12] = r_i, r_a, v_i, v_a (a.u.); device for ia_run,
                               host for ia_run_host                                                  */
@@ -126,9 +138,12 @@ typedef struct {
     double sum_ke, sum_ke2;     /* sum of ke_ion and ke_ion^2 over status == 0 trajectories (R16)    */
     uint64_t hist_ncoll[IA_HIST_BINS]; /* bin 0: n_coll = 0; bin b >= 1: 2^(b-1) <= n_coll < 2^b    */
     uint64_t t_first_idle_ns;   /* %globaltimer when the first lane found the work counter empty    */
-    uint64_t t_start_ns, t_end_ns; /* min / max %globaltimer over the kernel's warps                */
+    uint64_t t_start_ns, t_end_ns; /* first / last %globaltimer over the warps of both kernels       */
     uint64_t warn;              /* bit 0: 10|V(r0)| >= E_min (PAPER.md:28 asymptotic-start rule)     */
-    uint64_t reserved[16];
+    uint64_t n_handoff;         /* trajectories finished by the cooperative kernel after a hand-over */
+    uint64_t steps_coop;        /* attempted steps (incl. localisation) they took there              */
+    uint64_t t_bulk_end_ns;     /* last %globaltimer over the warps of the bulk kernel               */
+    uint64_t reserved[13];
 } ia_summary;
 
 typedef struct {
@@ -151,8 +166,15 @@ int ia_run_host(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *host_out
 /* Generator only (R1-R3): ic_dump is a DEVICE buffer [n][14]. */
 int ia_generate(ia_ctx *ctx, const ia_launch *launch, double *ic_dump, void *cuda_stream);
 
+/* Arithmetic variants of the verification entry points. */
+typedef enum {
+    IA_ARITH_NOFMA = 0,   /* every product and sum rounded separately ("fmad off")                  */
+    IA_ARITH_FMA = 1,     /* production arithmetic, one lane per trajectory (bulk kernel layout)     */
+    IA_ARITH_FMA_COOP = 2 /* production arithmetic, three lanes per trajectory (cooperative layout) */
+} ia_arith;
+
 /* Verification entry points (BASELINE.json north_star: "fixed-step mode built with fmad off").
- * use_fma = 0 runs the translation unit compiled with -fmad=false, 1 the production arithmetic.
+ * variant is an ia_arith; IA_ARITH_FMA and IA_ARITH_FMA_COOP give bit-identical results.
  *
  * ia_step_map: n independent single uncontrolled DP5(4) steps.  DEVICE arrays t_frac[n] (time folded
  * into [0,T_rf), R9), phase[n], y[n][12], h[n] in; ynew[n][12] and err[n] (the ode45 error norm of the
@@ -160,18 +182,29 @@ int ia_generate(ia_ctx *ctx, const ia_launch *launch, double *ic_dump, void *cud
  * ia_trace: nsteps uncontrolled steps of size h from y0[12] (HOST pointer) with rf phase `phase`;
  * states is a DEVICE buffer [nsteps+1][13] = (t, y) rows, row 0 the start. */
 int ia_step_map(ia_ctx *ctx, uint64_t n, const double *t_frac, const double *phase, const double *y,
-                const double *h, double *ynew, double *err, int use_fma, void *cuda_stream);
+                const double *h, double *ynew, double *err, int variant, void *cuda_stream);
 int ia_trace(ia_ctx *ctx, const double *y0_host, double phase, double h, uint32_t nsteps, double *states,
-             int use_fma, void *cuda_stream);
+             int variant, void *cuda_stream);
 
 /* Derived constants as the device sees them (host pointer, 16 doubles):
  * m_i, m_a, C4, C8, De, r_e, Omega, T_rf, thr, h_max, h_min, t_max, r0, r_coll, rtol, atol. */
 int ia_get_derived(const ia_ctx *ctx, double *out16);
 
 /* Launch geometry of ia_run on this ctx (host pointers): resident warps per SM, SM count,
- * registers per thread and local-memory (spill) bytes per thread of the persistent kernel. */
-int ia_get_kernel_info(const ia_ctx *ctx, int *warps_per_sm, int *n_sm, int *regs_per_thread,
+ * registers per thread and local-memory bytes per thread (the stack frame of the out-of-line
+ * generator; ptxas reports 0 spill bytes) of persistent kernel `kernel`: 0 bulk, 1 cooperative. */
+int ia_get_kernel_info(const ia_ctx *ctx, int kernel, int *warps_per_sm, int *n_sm, int *regs_per_thread,
                        int *local_bytes_per_thread);
+
+/* Hand-over threshold of IA_PATH_AUTO: a warp of the bulk kernel hands its running lanes over once
+ * the work counter is empty and at most `lanes` of them (0..32) still run; 0 = never (the default
+ * is 16: the cooperative kernel with ten trajectories per warp does the work of ~18 bulk lanes). */
+int ia_set_handoff(ia_ctx *ctx, int lanes);
+
+/* Device times of the most recent ia_run / ia_run_host of this ctx, from CUDA events the library
+ * records on the launch stream around its kernels: bulk kernel and cooperative kernel, in ms.
+ * Synchronises with the end of that run.  Host pointers. */
+int ia_get_last_timing(ia_ctx *ctx, double *bulk_ms, double *coop_ms);
 
 /* FP64 FMA peak microbenchmark (the roofline denominator): runs independent DFMA chains on every SM
  * of `cuda_device` for about `target_ms` and reports the sustained rate.  Host pointers.

@@ -23,11 +23,14 @@ LIB_PATH = _HERE / "libia_b200.so"
 
 IA_OK, IA_EINVAL, IA_ENOMEM, IA_ECUDA, IA_EDEVICE = 0, -1, -2, -3, -4
 IA_IC_EXPLICIT, IA_IC_GRID, IA_IC_PHILOX = 0, 1, 2
+IA_PATH_AUTO, IA_PATH_BULK_ONLY, IA_PATH_COOP_ONLY = 0, 1, 2
+IA_ARITH_NOFMA, IA_ARITH_FMA, IA_ARITH_FMA_COOP = 0, 1, 2
 IA_HIST_BINS = 32
 
 # every symbol include/ia.h declares (tests/test_cabi.py checks the library exports each of them)
 EXPORTS = ("ia_create", "ia_run", "ia_run_host", "ia_generate", "ia_step_map", "ia_trace", "ia_get_derived",
-           "ia_get_kernel_info", "ia_fp64_peak", "ia_destroy", "ia_strerror", "ia_last_error")
+           "ia_get_kernel_info", "ia_set_handoff", "ia_get_last_timing", "ia_fp64_peak", "ia_destroy", "ia_strerror",
+           "ia_last_error")
 
 
 class IaError(RuntimeError):
@@ -53,7 +56,7 @@ class ia_tol(C.Structure):
 
 class ia_launch(C.Structure):
     _fields_ = [("mode", C.c_int32), ("domain", C.c_int32), ("phase_mode", C.c_int32),
-                ("n_theta", C.c_uint32), ("n_phi", C.c_uint32), ("n", C.c_uint64),
+                ("n_theta", C.c_uint32), ("n_phi", C.c_uint32), ("path", C.c_int32), ("n", C.c_uint64),
                 ("y0", C.c_void_p), ("phase", C.c_void_p), ("phase0", C.c_double),
                 ("E_min_uK", C.c_double), ("E_max_uK", C.c_double), ("seed", C.c_uint64),
                 ("cell", C.c_uint32), ("first_index", C.c_uint64)]
@@ -70,7 +73,8 @@ SUMMARY_DTYPE = np.dtype([("n_done", "<u8"), ("n_status", "<u8", (5,)), ("n_comp
                           ("steps_acc", "<u8"), ("steps_rej", "<u8"), ("steps_loc", "<u8"),
                           ("sum_ke", "<f8"), ("sum_ke2", "<f8"), ("hist_ncoll", "<u8", (IA_HIST_BINS,)),
                           ("t_first_idle_ns", "<u8"), ("t_start_ns", "<u8"), ("t_end_ns", "<u8"),
-                          ("warn", "<u8"), ("reserved", "<u8", (16,))])
+                          ("warn", "<u8"), ("n_handoff", "<u8"), ("steps_coop", "<u8"), ("t_bulk_end_ns", "<u8"),
+                          ("reserved", "<u8", (13,))])
 RECORD_BYTES, SUMMARY_BYTES, IC_DUMP_COLS = 64, 512, 14
 assert RECORD_DTYPE.itemsize == RECORD_BYTES and SUMMARY_DTYPE.itemsize == SUMMARY_BYTES
 
@@ -100,7 +104,9 @@ def load() -> C.CDLL:
     L.ia_step_map.argtypes = [vp, C.c_uint64, vp, vp, vp, vp, vp, vp, C.c_int, vp]
     L.ia_trace.argtypes = [vp, dp, C.c_double, C.c_double, C.c_uint32, vp, C.c_int, vp]
     L.ia_get_derived.argtypes = [vp, dp]
-    L.ia_get_kernel_info.argtypes = [vp, ip, ip, ip, ip]
+    L.ia_get_kernel_info.argtypes = [vp, C.c_int, ip, ip, ip, ip]
+    L.ia_set_handoff.argtypes = [vp, C.c_int]
+    L.ia_get_last_timing.argtypes = [vp, dp, dp]
     L.ia_fp64_peak.argtypes = [C.c_int, C.c_double, dp, dp]
     L.ia_destroy.argtypes = [vp]
     L.ia_strerror.argtypes = [C.c_int]
@@ -157,6 +163,7 @@ def make_launch(launch, y0=None, phase=None) -> ia_launch:
     L = ia_launch()
     L.mode, L.domain, L.phase_mode = int(launch.mode), int(launch.domain), int(launch.phase_mode)
     L.n_theta, L.n_phi, L.n = int(launch.n_theta), int(launch.n_phi), int(launch.n)
+    L.path = int(getattr(launch, "path", 0))
     L.y0, L.phase = _ptr(y0), _ptr(phase)
     L.phase0, L.E_min_uK, L.E_max_uK = float(launch.phase0), float(launch.E_min_uK), float(launch.E_max_uK)
     L.seed, L.cell, L.first_index = int(launch.seed), int(launch.cell), int(launch.first_index)
@@ -197,17 +204,17 @@ def ia_generate(handle, launch: ia_launch, ic_dump, stream=None) -> None:
     _check(load().ia_generate(handle, C.byref(launch), _ptr(ic_dump), _stream_handle(stream)), handle)
 
 
-def ia_step_map(handle, n, t_frac, phase, y, h, ynew, err=None, use_fma: bool = True, stream=None) -> None:
+def ia_step_map(handle, n, t_frac, phase, y, h, ynew, err=None, variant: int = IA_ARITH_FMA, stream=None) -> None:
     _check(load().ia_step_map(handle, int(n), _ptr(t_frac), _ptr(phase), _ptr(y), _ptr(h), _ptr(ynew), _ptr(err),
-                              int(bool(use_fma)), _stream_handle(stream)), handle)
+                              int(variant), _stream_handle(stream)), handle)
 
 
-def ia_trace(handle, y0_host: np.ndarray, phase: float, h: float, nsteps: int, states, use_fma: bool = True,
+def ia_trace(handle, y0_host: np.ndarray, phase: float, h: float, nsteps: int, states, variant: int = IA_ARITH_FMA,
              stream=None) -> None:
     y0 = np.ascontiguousarray(y0_host, dtype=np.float64)
     assert y0.shape == (12,)
     _check(load().ia_trace(handle, y0.ctypes.data_as(C.POINTER(C.c_double)), float(phase), float(h), int(nsteps),
-                           _ptr(states), int(bool(use_fma)), _stream_handle(stream)), handle)
+                           _ptr(states), int(variant), _stream_handle(stream)), handle)
 
 
 _DERIVED_NAMES = ("m_i", "m_a", "C4", "C8", "De", "r_e", "Omega", "T_rf", "thr", "h_max", "h_min", "t_max", "r0",
@@ -220,11 +227,23 @@ def ia_get_derived(handle) -> dict:
     return dict(zip(_DERIVED_NAMES, list(out)))
 
 
-def ia_get_kernel_info(handle) -> dict:
+def ia_get_kernel_info(handle, kernel: int = 0) -> dict:
+    """kernel: 0 = bulk persistent kernel (one lane per trajectory), 1 = cooperative (three lanes)."""
     v = [C.c_int() for _ in range(4)]
-    _check(load().ia_get_kernel_info(handle, *[C.byref(x) for x in v]), handle)
+    _check(load().ia_get_kernel_info(handle, int(kernel), *[C.byref(x) for x in v]), handle)
     return {"warps_per_sm": v[0].value, "n_sm": v[1].value, "regs_per_thread": v[2].value,
             "local_bytes_per_thread": v[3].value}
+
+
+def ia_set_handoff(handle, lanes: int) -> None:
+    _check(load().ia_set_handoff(handle, int(lanes)), handle)
+
+
+def ia_get_last_timing(handle) -> dict:
+    """Device times (ms) of the two kernels of the most recent run on this ctx; synchronises with it."""
+    a, b = C.c_double(), C.c_double()
+    _check(load().ia_get_last_timing(handle, C.byref(a), C.byref(b)), handle)
+    return {"bulk_ms": a.value, "coop_ms": b.value}
 
 
 def ia_fp64_peak(device: int = 0, target_ms: float = 200.0) -> dict:
@@ -271,7 +290,14 @@ class Context:
 
     @property
     def kernel_info(self) -> dict:
-        return ia_get_kernel_info(self.handle)
+        return {"bulk": ia_get_kernel_info(self.handle, 0), "coop": ia_get_kernel_info(self.handle, 1)}
+
+    def set_handoff(self, lanes: int) -> None:
+        ia_set_handoff(self.handle, lanes)
+
+    @property
+    def last_timing(self) -> dict:
+        return ia_get_last_timing(self.handle)
 
     def alloc(self, n: int, ic_dump: bool = False):
         """(records uint8[n*64], summary uint8[512] zeroed, ic_dump float64[n,14] or None) on the device."""
@@ -320,7 +346,7 @@ class Context:
         torch.cuda.synchronize(self.device)
         return ic.cpu().numpy()[:n]
 
-    def step_map(self, t_frac, phase, y, h, use_fma: bool = True):
+    def step_map(self, t_frac, phase, y, h, variant: int = IA_ARITH_FMA):
         """n single uncontrolled steps: returns (ynew[n,12], err[n]) as numpy."""
         import torch
         dev = f"cuda:{self.device}"
@@ -330,15 +356,15 @@ class Context:
         d = [torch.as_tensor(a).to(dev) for a in (bc(t_frac), bc(phase), y, bc(h))]
         ynew = torch.empty((max(n, 1), 12), dtype=torch.float64, device=dev)
         err = torch.empty(max(n, 1), dtype=torch.float64, device=dev)
-        ia_step_map(self.handle, n, d[0], d[1], d[2], d[3], ynew, err, use_fma)
+        ia_step_map(self.handle, n, d[0], d[1], d[2], d[3], ynew, err, variant)
         torch.cuda.synchronize(self.device)
         return ynew.cpu().numpy()[:n], err.cpu().numpy()[:n]
 
-    def trace(self, y0, phase: float, h: float, nsteps: int, use_fma: bool = True) -> np.ndarray:
+    def trace(self, y0, phase: float, h: float, nsteps: int, variant: int = IA_ARITH_FMA) -> np.ndarray:
         """nsteps uncontrolled steps of size h: (t, y) rows [nsteps+1, 13] as numpy."""
         import torch
         st = torch.empty((nsteps + 1, 13), dtype=torch.float64, device=f"cuda:{self.device}")
-        ia_trace(self.handle, np.asarray(y0, dtype=np.float64), phase, h, nsteps, st, use_fma)
+        ia_trace(self.handle, np.asarray(y0, dtype=np.float64), phase, h, nsteps, st, variant)
         torch.cuda.synchronize(self.device)
         return st.cpu().numpy()
 

@@ -19,20 +19,32 @@ const double PI = 3.14159265358979323846;
 
 } // namespace
 
+struct IaKernelInfo {
+    int blocks_per_sm = 0, threads_per_block = 0, regs = 0, local_bytes = 0;
+};
+
 struct ia_ctx {
     int device = 0;
     IaParams P;
     double derived[16];
-    unsigned long long *counters = nullptr; /* ring of work counters, one per in-flight launch */
+    /* per-launch scratch, a ring so that launches queued behind one another on a stream do not share:
+     * slot = [work counter of the bulk kernel, number handed over, work counter of the cooperative kernel, pad] */
+    unsigned long long *counters = nullptr;
     unsigned counter_next = 0;
-    int n_sm = 0, blocks_per_sm = 0, threads_per_block = 0, regs = 0, local_bytes = 0;
+    IaHand *queue = nullptr; /* hand-over queue: one entry per lane of a full bulk grid */
+    size_t queue_cap = 0;
+    int handoff_lanes = 16;
+    int n_sm = 0;
+    IaKernelInfo kinfo[2]; /* 0 bulk, 1 cooperative */
+    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr}; /* start, between the kernels, end of the last run */
+    bool timed = false;
     /* staging for ia_run_host */
     void *stage = nullptr;
     size_t stage_bytes = 0;
     std::string err;
 };
 
-#define IA_COUNTER_RING 1024
+#define IA_COUNTER_RING 256 /* slots of 4 x u64 */
 
 static int fail_cuda(ia_ctx *c, const char *what, cudaError_t e) {
     if (c) c->err = std::string(what) + ": " + cudaGetErrorString(e);
@@ -104,7 +116,7 @@ int ia_create(ia_ctx **out, const ia_species *sp, const ia_trap *tr, double De_K
     P.C8 = P.C4 * P.C4 / (4.0 * P.De);
     P.r_e = std::pow(2.0 * P.C8 / P.C4, 0.25);
     P.c8x8 = 8.0 * P.C8;
-    P.c4x4 = 4.0 * P.C4;
+    P.neg_c4x4 = -4.0 * P.C4;
     P.omega = tr->omega_rf_au;
     P.T_rf = 2.0 * PI / P.omega;
     for (int k = 0; k < 3; ++k) {
@@ -114,7 +126,6 @@ int ia_create(ia_ctx **out, const ia_species *sp, const ia_trap *tr, double De_K
     P.rtol = T.rtol;
     P.atol = T.atol;
     P.thr = T.atol / T.rtol;
-    P.inv_rtol = 1.0 / T.rtol;
     P.h_max = T.h_max_rf * P.T_rf;
     P.h_min = std::ldexp(P.T_rf, -40);
     P.t_max_rf = T.t_max_rf;
@@ -130,16 +141,22 @@ int ia_create(ia_ctx **out, const ia_species *sp, const ia_trap *tr, double De_K
                           P.thr, P.h_max, P.h_min, P.t_max, P.r0, P.r_coll, P.rtol, P.atol};
     std::memcpy(c->derived, d, sizeof(d));
 
-    cudaError_t e = cudaSetDevice(cuda_device);
-    if (e == cudaSuccess) e = cudaMalloc(&c->counters, IA_COUNTER_RING * sizeof(unsigned long long));
-    if (e == cudaSuccess)
-        e = ia_persistent_info(cuda_device, &c->blocks_per_sm, &c->threads_per_block, &c->regs, &c->local_bytes);
-    if (e != cudaSuccess) {
-        if (c->counters) cudaFree(c->counters);
-        delete c;
-        return e == cudaErrorMemoryAllocation ? IA_ENOMEM : IA_ECUDA;
-    }
     c->n_sm = prop.multiProcessorCount;
+    cudaError_t e = cudaSetDevice(cuda_device);
+    if (e == cudaSuccess) e = cudaMalloc(&c->counters, IA_COUNTER_RING * 4 * sizeof(unsigned long long));
+    for (int k = 0; k < 2 && e == cudaSuccess; ++k)
+        e = ia_persistent_info(k == 0 ? 1 : 3, &c->kinfo[k].blocks_per_sm, &c->kinfo[k].threads_per_block,
+                               &c->kinfo[k].regs, &c->kinfo[k].local_bytes);
+    if (e == cudaSuccess) {
+        c->queue_cap = (size_t)c->n_sm * c->kinfo[0].blocks_per_sm * c->kinfo[0].threads_per_block;
+        e = cudaMalloc(&c->queue, c->queue_cap * sizeof(IaHand));
+    }
+    for (int k = 0; k < 3 && e == cudaSuccess; ++k) e = cudaEventCreate(&c->ev[k]);
+    if (e != cudaSuccess) {
+        const int rc = e == cudaErrorMemoryAllocation ? IA_ENOMEM : IA_ECUDA;
+        ia_destroy(c);
+        return rc;
+    }
     *out = c;
     return IA_OK;
 }
@@ -148,7 +165,10 @@ int ia_destroy(ia_ctx *ctx) {
     if (!ctx) return IA_EINVAL;
     cudaSetDevice(ctx->device);
     if (ctx->counters) cudaFree(ctx->counters);
+    if (ctx->queue) cudaFree(ctx->queue);
     if (ctx->stage) cudaFree(ctx->stage);
+    for (int k = 0; k < 3; ++k)
+        if (ctx->ev[k]) cudaEventDestroy(ctx->ev[k]);
     delete ctx;
     return IA_OK;
 }
@@ -159,13 +179,34 @@ int ia_get_derived(const ia_ctx *ctx, double *out16) {
     return IA_OK;
 }
 
-int ia_get_kernel_info(const ia_ctx *ctx, int *warps_per_sm, int *n_sm, int *regs_per_thread,
+int ia_get_kernel_info(const ia_ctx *ctx, int kernel, int *warps_per_sm, int *n_sm, int *regs_per_thread,
                        int *local_bytes_per_thread) {
-    if (!ctx) return IA_EINVAL;
-    if (warps_per_sm) *warps_per_sm = ctx->blocks_per_sm * ctx->threads_per_block / 32;
+    if (!ctx || kernel < 0 || kernel > 1) return IA_EINVAL;
+    const IaKernelInfo &k = ctx->kinfo[kernel];
+    if (warps_per_sm) *warps_per_sm = k.blocks_per_sm * k.threads_per_block / 32;
     if (n_sm) *n_sm = ctx->n_sm;
-    if (regs_per_thread) *regs_per_thread = ctx->regs;
-    if (local_bytes_per_thread) *local_bytes_per_thread = ctx->local_bytes;
+    if (regs_per_thread) *regs_per_thread = k.regs;
+    if (local_bytes_per_thread) *local_bytes_per_thread = k.local_bytes;
+    return IA_OK;
+}
+
+int ia_set_handoff(ia_ctx *ctx, int lanes) {
+    if (!ctx || lanes < 0 || lanes > 32) return IA_EINVAL;
+    ctx->handoff_lanes = lanes;
+    return IA_OK;
+}
+
+int ia_get_last_timing(ia_ctx *ctx, double *bulk_ms, double *coop_ms) {
+    if (!ctx || !bulk_ms || !coop_ms) return IA_EINVAL;
+    if (!ctx->timed) return fail_inval(ctx, "no run has been timed on this ctx yet");
+    cudaError_t e = cudaSetDevice(ctx->device);
+    if (e == cudaSuccess) e = cudaEventSynchronize(ctx->ev[2]);
+    float a = 0.f, b = 0.f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&a, ctx->ev[0], ctx->ev[1]);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&b, ctx->ev[1], ctx->ev[2]);
+    if (e != cudaSuccess) return fail_cuda(ctx, "ia_get_last_timing", e);
+    *bulk_ms = a;
+    *coop_ms = b;
     return IA_OK;
 }
 
@@ -178,6 +219,8 @@ static int make_gen(ia_ctx *ctx, const ia_launch *L, IaGen *G, unsigned long lon
     *warn = 0;
     if (L->mode != IA_IC_EXPLICIT && L->mode != IA_IC_GRID && L->mode != IA_IC_PHILOX)
         return fail_inval(ctx, "launch.mode is not an ia_ic_mode");
+    if (L->path != IA_PATH_AUTO && L->path != IA_PATH_BULK_ONLY && L->path != IA_PATH_COOP_ONLY)
+        return fail_inval(ctx, "launch.path is not an ia_path");
     G->mode = L->mode;
     G->n = L->n;
     G->first_index = L->first_index;
@@ -225,9 +268,11 @@ static int make_gen(ia_ctx *ctx, const ia_launch *L, IaGen *G, unsigned long lon
     return IA_OK;
 }
 
-static int grid_for(const ia_ctx *ctx, unsigned long long n) {
-    const unsigned long long full = (unsigned long long)ctx->n_sm * ctx->blocks_per_sm;
-    const unsigned long long need = (n + ctx->threads_per_block - 1) / ctx->threads_per_block;
+/* blocks of persistent kernel k (0 bulk: 32 trajectories per warp; 1 cooperative: 10) for n trajectories */
+static int grid_for(const ia_ctx *ctx, int k, unsigned long long n) {
+    const unsigned long long full = (unsigned long long)ctx->n_sm * ctx->kinfo[k].blocks_per_sm;
+    const unsigned long long per = k == 0 ? 32ull : 10ull;
+    const unsigned long long need = (n + per - 1) / per;
     return (int)(need < full ? need : full);
 }
 
@@ -245,15 +290,48 @@ int ia_run(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *outputs, void
     cudaStream_t st = (cudaStream_t)cuda_stream;
     cudaError_t e = cudaSetDevice(ctx->device);
     if (e != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", e);
-    unsigned long long *counter = ctx->counters + (ctx->counter_next++ % IA_COUNTER_RING);
-    e = cudaMemsetAsync(counter, 0, sizeof(unsigned long long), st);
+    unsigned long long *scratch = ctx->counters + 4 * (size_t)(ctx->counter_next++ % IA_COUNTER_RING);
+    e = cudaMemsetAsync(scratch, 0, 4 * sizeof(unsigned long long), st);
     if (e != cudaSuccess) return fail_cuda(ctx, "cudaMemsetAsync(counter)", e);
     IaOut O;
     O.records = outputs->records;
     O.summary = outputs->summary;
     O.ic_dump = outputs->ic_dump;
-    e = ia_launch_persistent(ctx->P, G, O, counter, warn, grid_for(ctx, G.n), st);
+    const bool coop_only = launch->path == IA_PATH_COOP_ONLY;
+    const bool handoff = launch->path == IA_PATH_AUTO && ctx->handoff_lanes > 0;
+    IaSched S;
+    std::memset(&S, 0, sizeof(S));
+    S.counter = scratch;
+    S.warn = warn;
+    e = cudaEventRecord(ctx->ev[0], st);
+    if (e != cudaSuccess) return fail_cuda(ctx, "cudaEventRecord", e);
+    if (coop_only) {
+        e = ia_launch_persistent(3, ctx->P, G, O, S, grid_for(ctx, 1, G.n), st);
+        if (e == cudaSuccess) e = cudaEventRecord(ctx->ev[1], st);
+    } else {
+        if (handoff) {
+            S.q_out = ctx->queue;
+            S.n_out = scratch + 1;
+            S.handoff_lanes = ctx->handoff_lanes;
+        }
+        const int blocks = grid_for(ctx, 0, G.n);
+        e = ia_launch_persistent(1, ctx->P, G, O, S, blocks, st);
+        if (e == cudaSuccess) e = cudaEventRecord(ctx->ev[1], st);
+        if (e == cudaSuccess && handoff) {
+            /* the straggler kernel resumes what the bulk kernel queued; it is enqueued behind it on the same
+             * stream with a grid that can hold every lane the bulk grid could have handed over */
+            IaSched S5;
+            std::memset(&S5, 0, sizeof(S5));
+            S5.counter = scratch + 2;
+            S5.q_in = ctx->queue;
+            S5.n_in = scratch + 1;
+            const unsigned long long most = (unsigned long long)blocks * (unsigned long long)ctx->handoff_lanes;
+            e = ia_launch_persistent(3, ctx->P, G, O, S5, grid_for(ctx, 1, most), st);
+        }
+    }
+    if (e == cudaSuccess) e = cudaEventRecord(ctx->ev[2], st);
     if (e != cudaSuccess) return fail_cuda(ctx, "persistent kernel launch", e);
+    ctx->timed = true;
     return IA_OK;
 }
 
@@ -331,32 +409,33 @@ int ia_generate(ia_ctx *ctx, const ia_launch *launch, double *ic_dump, void *cud
     return IA_OK;
 }
 
+static bool bad_variant(int v) { return v != IA_ARITH_NOFMA && v != IA_ARITH_FMA && v != IA_ARITH_FMA_COOP; }
+
 int ia_step_map(ia_ctx *ctx, uint64_t n, const double *t_frac, const double *phase, const double *y, const double *h,
-                double *ynew, double *err, int use_fma, void *cuda_stream) {
+                double *ynew, double *err, int variant, void *cuda_stream) {
     if (!ctx) return IA_EINVAL;
     ctx->err.clear();
     if (n == 0) return IA_OK;
     if (!t_frac || !phase || !y || !h || !ynew) return fail_inval(ctx, "ia_step_map: NULL array");
+    if (bad_variant(variant)) return fail_inval(ctx, "ia_step_map: variant is not an ia_arith");
     cudaError_t e = cudaSetDevice(ctx->device);
     if (e == cudaSuccess)
-        e = use_fma ? ia_launch_step_map_fma(ctx->P, n, t_frac, phase, y, h, ynew, err, (cudaStream_t)cuda_stream)
-                    : ia_launch_step_map_nofma(ctx->P, n, t_frac, phase, y, h, ynew, err, (cudaStream_t)cuda_stream);
+        e = ia_launch_step_map(variant, ctx->P, n, t_frac, phase, y, h, ynew, err, (cudaStream_t)cuda_stream);
     if (e != cudaSuccess) return fail_cuda(ctx, "step-map launch", e);
     return IA_OK;
 }
 
-int ia_trace(ia_ctx *ctx, const double *y0_host, double phase, double h, uint32_t nsteps, double *states, int use_fma,
+int ia_trace(ia_ctx *ctx, const double *y0_host, double phase, double h, uint32_t nsteps, double *states, int variant,
              void *cuda_stream) {
     if (!ctx) return IA_EINVAL;
     ctx->err.clear();
     if (!y0_host || !states) return fail_inval(ctx, "ia_trace: NULL array");
     if (!std::isfinite(phase) || !std::isfinite(h)) return fail_inval(ctx, "ia_trace: non-finite phase or h");
+    if (bad_variant(variant)) return fail_inval(ctx, "ia_trace: variant is not an ia_arith");
     IaY12 y0;
     std::memcpy(y0.y, y0_host, sizeof(y0.y));
     cudaError_t e = cudaSetDevice(ctx->device);
-    if (e == cudaSuccess)
-        e = use_fma ? ia_launch_trace_fma(ctx->P, y0, phase, h, nsteps, states, (cudaStream_t)cuda_stream)
-                    : ia_launch_trace_nofma(ctx->P, y0, phase, h, nsteps, states, (cudaStream_t)cuda_stream);
+    if (e == cudaSuccess) e = ia_launch_trace(variant, ctx->P, y0, phase, h, nsteps, states, (cudaStream_t)cuda_stream);
     if (e != cudaSuccess) return fail_cuda(ctx, "trace launch", e);
     return IA_OK;
 }

@@ -2,134 +2,38 @@
  * ia_dev.cuh -- device arithmetic of the ion+atom propagator: right-hand side, one Dormand-Prince
  * 5(4) attempt in second-order (Nystrom-collapsed) form, error norm, fifth root, cosine.
  *
- * Included by ia_kernels.cu (production arithmetic, FMA contraction on) and by ia_nofma.cu
- * (compiled with -fmad=false: every a*b+c below is two rounded operations there; only the explicit
- * fma() calls in the reciprocal / range reduction stay fused).  Shares nothing with oracle/.
- *
- * Method (Eq. 1-2, PAPER.md:20,26 refs [22,23]):
+ * Shares nothing with oracle/.  Method (Eq. 1-2, PAPER.md:20,26 refs [22,23];
+ * DESIGN.md "Kernels"):
  *   y = (x, v) with x = (r_i, r_a), v = (v_i, v_a); dx/dt = v, dv/dt = A(t, x) -- the force does not
  *   depend on velocity, so the 7-stage DP5(4) step collapses exactly to
  *       X_s   = x + (h c_s) v + h^2 sum_l abar_sl A_l,      abar = a.a
  *       v_new = v + h sum_l b_l A_l,        x_new = X_7
  *       e_x   = h^2 sum_l ebar_l A_l,       e_v = h sum_l E_l A_l,   ebar = E.a,  E = b - bhat
  *   (sum_l E_l = 0 removes the v term of e_x).  The stage velocities V_2..V_6 are never formed.
+ *
+ * Two template parameters run through everything:
+ *   LPT   lanes per trajectory.  1: one lane holds all six (x, v) component pairs (the throughput
+ *         layout of the bulk kernel).  3: lane k of a group of three holds axis k of the ion and of
+ *         the atom; the separation vector is gathered with warp shuffles (the latency layout of the
+ *         straggler kernel: a third of the FP64 instructions per lane and step).
+ *   FUSED true: production arithmetic, every a*b+c below written as an explicit fma().
+ *         false: the same expressions with a separately rounded product and sum (the "fmad off"
+ *         verification variant of BASELINE.json's north_star).
+ * The translation units are compiled with -fmad=false, so the compiler never contracts on its own:
+ * the sequence of IEEE operations per component is fixed by this source alone, and the two layouts
+ * give BIT-IDENTICAL results (every cross-component sum is taken in the one order d0,d1,d2; every
+ * comparison tree in the one order written here).  tests/test_gpu_parity.py checks that bitwise.
  */
 #pragma once
 #include <stdint.h>
 
-struct IaParams {
-    /* pair potential and masses */
-    double inv_m_a;     /*  1/m_a                       */
-    double neg_inv_m_i; /* -1/m_i                       */
-    double m_i, m_a;
-    double c8x8, c4x4;  /* 8 C8, 4 C4                   */
-    /* trap: A_i,k += (ka_k + kq_k cos(Omega t + phase)) r_i,k */
-    double ka[3];       /* -a_k Omega^2/4               */
-    double kq[3];       /* -q_k Omega^2/2               */
-    double omega, T_rf;
-    /* controller (reading R5) */
-    double rtol, thr, inv_rtol;
-    double h_max, h_min, t_max_rf, t_max;
-    double h0_scale;    /* 0.8 rtol^(1/5) (divides rho) */
-    /* events / termination (R6, R7) */
-    double r0, r0sq, rcsq, loc_tol; /* loc_tol = 1e-13 r0^2 */
-    double C4, C8, De, r_e, r_coll, atol;
-    unsigned long long max_steps;
-};
-
-#define IA_DEV __device__ __forceinline__
-
-/* ---- small FP64 helpers ------------------------------------------------------------------- */
-
-/* 1/x for normal, finite, non-zero x: MUFU.RCP64H seed (rel. err <= 2^-23) and one third-order
- * correction y <- y + y(e + e^2), e = 1 - x y  (error e^3 ~ 2^-69, result within ~1 ulp).
- * x = 0, inf or NaN gives NaN -- the callers rely on that to flag non-finite states. */
-IA_DEV double ia_rcp(double x) {
-    double y;
-    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-    const double e = fma(-x, y, 1.0);
-    const double e2 = fma(e, e, e);
-    return fma(y, e2, y);
-}
-
-/* x^(-1/5) for x in [1e-30, 1e30]: FP32 MUFU seed (lg2/ex2, rel. err ~1e-6) and two Newton steps
- * y <- y (6 - x y^5)/5 (rel. err -> 3e-12 -> ~3e-23). */
-IA_DEV double ia_inv_fifth_root(double x) {
-    const float xf = (float)x;
-    float lf;
-    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(lf) : "f"(xf));
-    float sf;
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(sf) : "f"(-0.2f * lf));
-    double y = (double)sf;
-#pragma unroll
-    for (int it = 0; it < 2; ++it) {
-        const double y2 = y * y;
-        const double y4 = y2 * y2;
-        const double y5 = y4 * y;
-        const double t = fma(-x, y5, 6.0);
-        y = (0.2 * y) * t;
-    }
-    return y;
-}
-
-/* cos(arg) for arg in about [-4 pi, 8 pi] (the callers keep time folded, reading R9):
- * n = rint(arg/pi), r = arg - n pi (two-constant Cody-Waite with exact fma products),
- * cos(arg) = (-1)^n cos(r), |r| <= pi/2, Taylor polynomial in r^2 through r^22
- * (truncation (pi/2)^24/24! = 8e-20; absolute error ~1e-16). */
-IA_DEV double ia_cos_folded(double arg) {
-    const double MAGIC = 6755399441055744.0; /* 1.5 * 2^52: adding it rounds to nearest integer */
-    const double nf = fma(arg, 0.31830988618379067154, MAGIC);
-    const double n = nf - MAGIC;
-    double r = fma(-n, 3.14159265358979311600e+00, arg);
-    r = fma(-n, 1.22464679914735317723e-16, r);
-    const double z = r * r;
-    double p = -1.0 / 1124000727777607680000.0;          /* -1/22! */
-    p = p * z + 1.0 / 2432902008176640000.0;             /*  1/20! */
-    p = p * z - 1.0 / 6402373705728000.0;                /* -1/18! */
-    p = p * z + 1.0 / 20922789888000.0;                  /*  1/16! */
-    p = p * z - 1.0 / 87178291200.0;                     /* -1/14! */
-    p = p * z + 1.0 / 479001600.0;                       /*  1/12! */
-    p = p * z - 1.0 / 3628800.0;                         /* -1/10! */
-    p = p * z + 1.0 / 40320.0;                           /*  1/8!  */
-    p = p * z - 1.0 / 720.0;                             /* -1/6!  */
-    p = p * z + 1.0 / 24.0;                              /*  1/4!  */
-    p = p * z - 0.5;                                     /* -1/2!  */
-    p = p * z + 1.0;
-    /* flip the sign when n is odd: the integer n sits in the low word of nf */
-    const int lo = __double2loint(nf);
-    const int hi = __double2hiint(p) ^ (lo << 31);
-    return __hiloint2double(hi, __double2loint(p));
-}
-
-/* ---- right-hand side (reading O1) ------------------------------------------ */
-
-/* Accelerations A[0..2] (ion) and A[3..5] (atom) at positions X = (r_i, r_a), with c = cos(Omega t
- * + phase).  Also returns r^2 = |r_a - r_i|^2 and the scalar s = u^3 (8 C8 u^2 - 4 C4), u = 1/r^2:
- * force on the atom = -dV/dr d/r = s d. */
-IA_DEV void ia_accel(const IaParams &P, const double (&X)[6], double c, double (&A)[6], double &r2, double &s) {
-    const double d0 = X[3] - X[0], d1 = X[4] - X[1], d2 = X[5] - X[2];
-    r2 = d0 * d0 + d1 * d1 + d2 * d2;
-    const double u = ia_rcp(r2);
-    const double u2 = u * u;
-    const double t = P.c8x8 * u2 - P.c4x4;
-    s = (u2 * u) * t;
-    const double sa = s * P.inv_m_a;
-    const double si = s * P.neg_inv_m_i;
-    A[3] = sa * d0;
-    A[4] = sa * d1;
-    A[5] = sa * d2;
-    A[0] = si * d0 + (P.ka[0] + P.kq[0] * c) * X[0];
-    A[1] = si * d1 + (P.ka[1] + P.kq[1] * c) * X[1];
-    A[2] = si * d2 + (P.ka[2] + P.kq[2] * c) * X[2];
-}
-
-/* ---- Dormand-Prince 5(4), ref [22] ------------------------------------------- */
+/* ---- Dormand-Prince 5(4), ref [22], exact rationals ------------------------------ */
 /* nodes */
 #define IA_C2 (1.0 / 5.0)
 #define IA_C3 (3.0 / 10.0)
 #define IA_C4 (4.0 / 5.0)
 #define IA_C5 (8.0 / 9.0)
-/* abar = a.a (exact rationals; tests/test_host_logic.py re-derives them from the tableau) */
+/* abar = a.a (tests/test_host_logic.py re-derives them from the tableau) */
 #define IA_AB31 (9.0 / 200.0)
 #define IA_AB41 (-12.0 / 25.0)
 #define IA_AB42 (4.0 / 5.0)
@@ -164,8 +68,187 @@ IA_DEV void ia_accel(const IaParams &P, const double (&X)[6], double c, double (
 #define IA_EB5 (-4617.0 / 1356800.0)
 #define IA_EB6 (-11.0 / 3360.0)
 
+struct IaParams {
+    /* pair potential and masses */
+    double inv_m_a;     /*  1/m_a                       */
+    double neg_inv_m_i; /* -1/m_i                       */
+    double m_i, m_a;
+    double c8x8, neg_c4x4; /* 8 C8, -4 C4              */
+    /* trap: A_i,k += (ka_k + kq_k cos(Omega t + phase)) r_i,k */
+    double ka[3];       /* -a_k Omega^2/4               */
+    double kq[3];       /* -q_k Omega^2/2               */
+    double omega, T_rf;
+    /* controller (reading R5) */
+    double rtol, thr;
+    double h_max, h_min, t_max_rf, t_max;
+    double h0_scale;    /* 0.8 rtol^(1/5) (divides rho) */
+    /* events / termination (R6, R7) */
+    double r0, r0sq, rcsq, loc_tol; /* loc_tol = 1e-13 r0^2 */
+    double C4, C8, De, r_e, r_coll, atol;
+    unsigned long long max_steps;
+};
+
+#define IA_DEV __device__ __forceinline__
+#define IA_FULL 0xffffffffu
+
+/* ---- small FP64 helpers ------------------------------------------------------------------------ */
+
+template <bool FUSED>
+IA_DEV double ia_fma(double a, double b, double c) {
+    return FUSED ? fma(a, b, c) : __dadd_rn(__dmul_rn(a, b), c);
+}
+
+/* 1/x for normal, finite, non-zero x: MUFU.RCP64H seed (rel. err <= 2^-23) and one third-order
+ * correction y <- y + y(e + e^2), e = 1 - x y  (error e^3 ~ 2^-69, result within ~1 ulp).
+ * x = 0, inf or NaN gives NaN -- the callers rely on that to flag non-finite states.
+ * (The three fma here stay fused in both variants: they are the definition of this reciprocal.) */
+IA_DEV double ia_rcp(double x) {
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double e = fma(-x, y, 1.0);
+    const double e2 = fma(e, e, e);
+    return fma(y, e2, y);
+}
+
+/* x^(-1/5) for x in [1e-30, 1e30]: FP32 MUFU seed (lg2/ex2, rel. err ~1e-6) and two Newton steps
+ * y <- y (6 - x y^5)/5 (rel. err -> 3e-12 -> ~3e-23). */
+IA_DEV double ia_inv_fifth_root(double x) {
+    const float xf = (float)x;
+    float lf;
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(lf) : "f"(xf));
+    float sf;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(sf) : "f"(-0.2f * lf));
+    double y = (double)sf;
+#pragma unroll
+    for (int it = 0; it < 2; ++it) {
+        const double y2 = y * y;
+        const double y4 = y2 * y2;
+        const double y5 = y4 * y;
+        const double t = fma(-x, y5, 6.0);
+        y = (0.2 * y) * t;
+    }
+    return y;
+}
+
+/* cos(arg) for arg in about [-4 pi, 8 pi] (the callers keep time folded, reading R9):
+ * n = rint(arg/pi), r = arg - n pi (two-constant Cody-Waite with exact fma products),
+ * cos(arg) = (-1)^n cos(r), |r| <= pi/2, Taylor polynomial in z = r^2 through r^22
+ * (truncation (pi/2)^24/24! = 8e-20; absolute error ~1e-16). */
+IA_DEV double ia_cos_folded(double arg) {
+    const double MAGIC = 6755399441055744.0; /* 1.5 * 2^52: adding it rounds to nearest integer */
+    const double nf = fma(arg, 0.31830988618379067154, MAGIC);
+    const double n = nf - MAGIC;
+    double r = fma(-n, 3.14159265358979311600e+00, arg);
+    r = fma(-n, 1.22464679914735317723e-16, r);
+    const double z = r * r;
+    double p = -1.0 / 1124000727777607680000.0;         /* -1/22! */
+    p = fma(p, z, 1.0 / 2432902008176640000.0);         /*  1/20! */
+    p = fma(p, z, -1.0 / 6402373705728000.0);           /* -1/18! */
+    p = fma(p, z, 1.0 / 20922789888000.0);              /*  1/16! */
+    p = fma(p, z, -1.0 / 87178291200.0);                /* -1/14! */
+    p = fma(p, z, 1.0 / 479001600.0);                   /*  1/12! */
+    p = fma(p, z, -1.0 / 3628800.0);                    /* -1/10! */
+    p = fma(p, z, 1.0 / 40320.0);                       /*  1/8!  */
+    p = fma(p, z, -1.0 / 720.0);                        /* -1/6!  */
+    p = fma(p, z, 1.0 / 24.0);                          /*  1/4!  */
+    p = fma(p, z, -0.5);                                /* -1/2!  */
+    p = fma(p, z, 1.0);
+    /* flip the sign when n is odd: the integer n sits in the low word of nf */
+    const int lo = __double2loint(nf);
+    const int hi = __double2hiint(p) ^ (lo << 31);
+    return __hiloint2double(hi, __double2loint(p));
+}
+
+/* Scheduling fence without an instruction: makes `x` look redefined once `after` is known, so that the
+ * chain starting from x is not hoisted above the computation of `after` (register pressure only). */
+#define IA_TIE(x, after) asm volatile("" : "+d"(x) : "d"(after))
+
+/* ---- lane layout -------------------------------------------------------------------------------- */
+
+/* What a lane knows about its place: with LPT = 1 a lane is its own group and holds axes 0,1,2;
+ * with LPT = 3 lanes 3g, 3g+1, 3g+2 form group g and lane 3g+k holds axis k (lanes 30, 31 idle). */
+template <int LPT>
+struct IaLane {
+    static constexpr int NA = 3 / LPT; /* axes held by this lane */
+    unsigned gbase;                    /* first lane of the group */
+    unsigned axis0;                    /* global axis of local axis 0 */
+    double ka[1], kq[1];               /* LPT = 3: trap constants of the lane's axis (LPT = 1 reads P.ka/P.kq) */
+    bool valid;                        /* lane belongs to a complete group */
+    bool leader;                       /* first lane of its group */
+};
+
+template <int LPT>
+IA_DEV IaLane<LPT> ia_make_lane(const IaParams &P, unsigned lane) {
+    IaLane<LPT> L;
+    if (LPT == 1) {
+        L.gbase = lane;
+        L.axis0 = 0;
+        L.valid = true;
+        L.leader = true;
+        L.ka[0] = 0.0;
+        L.kq[0] = 0.0;
+    } else {
+        const unsigned g = lane / 3u, k = lane - 3u * g;
+        L.gbase = 3u * g;
+        L.axis0 = k;
+        L.valid = lane < 30u;
+        L.leader = (k == 0u) && L.valid;
+        L.ka[0] = (k == 0u) ? P.ka[0] : (k == 1u) ? P.ka[1] : P.ka[2];
+        L.kq[0] = (k == 0u) ? P.kq[0] : (k == 1u) ? P.kq[1] : P.kq[2];
+    }
+    return L;
+}
+
+/* full 3-vector from the local axes (every lane of the warp must call this together when LPT = 3) */
+template <int LPT>
+IA_DEV void ia_gather3(const IaLane<LPT> &L, const double (&loc)[3 / LPT], double (&full)[3]) {
+    if (LPT == 1) {
+#pragma unroll
+        for (int a = 0; a < 3 / LPT; ++a) full[a] = loc[a];
+    } else {
+#pragma unroll
+        for (int j = 0; j < 3; ++j) full[j] = __shfl_sync(IA_FULL, loc[0], (int)(L.gbase + j));
+    }
+}
+
+/* canonical dot product of two gathered 3-vectors: fma(a2,b2, fma(a1,b1, a0 b0)) */
+template <bool FUSED>
+IA_DEV double ia_dot3(const double (&a)[3], const double (&b)[3]) {
+    return ia_fma<FUSED>(a[2], b[2], ia_fma<FUSED>(a[1], b[1], a[0] * b[0]));
+}
+
+/* ---- right-hand side (reading O1) ------------------------------------------------ */
+
+/* Accelerations of the local axes at positions (Xi, Xa), with c = cos(Omega t + phase).
+ * Also returns the gathered separation d = r_a - r_i, r^2 = |d|^2 and s = u^3 (8 C8 u^2 - 4 C4),
+ * u = 1/r^2: force on the atom = -dV/dr d/r = s d. */
+template <int LPT, bool FUSED>
+IA_DEV void ia_accel(const IaParams &P, const IaLane<LPT> &L, const double (&Xi)[3 / LPT], const double (&Xa)[3 / LPT],
+                     double c, double (&Ai)[3 / LPT], double (&Aa)[3 / LPT], double (&D)[3], double &r2, double &s) {
+    constexpr int NA = 3 / LPT;
+    double d[NA];
+#pragma unroll
+    for (int a = 0; a < NA; ++a) d[a] = Xa[a] - Xi[a];
+    ia_gather3<LPT>(L, d, D);
+    r2 = ia_dot3<FUSED>(D, D);
+    const double u = ia_rcp(r2);
+    const double u2 = u * u;
+    const double t = ia_fma<FUSED>(P.c8x8, u2, P.neg_c4x4);
+    s = (u2 * u) * t;
+    const double sa = s * P.inv_m_a;
+    const double si = s * P.neg_inv_m_i;
+#pragma unroll
+    for (int a = 0; a < NA; ++a) {
+        Aa[a] = sa * d[a];
+        const double trap = (LPT == 1) ? ia_fma<FUSED>(P.kq[a], c, P.ka[a]) : ia_fma<FUSED>(L.kq[0], c, L.ka[0]);
+        Ai[a] = ia_fma<FUSED>(si, d[a], trap * Xi[a]);
+    }
+}
+
+/* ---- error norm (reading R5) --------------------------------------------------------------------- */
+
 struct IaErr {
-    double num, den; /* err = num/den = max_i |e_i| / max(|y_i|, |ynew_i|, thr)   (reading R5) */
+    double num, den; /* err = num/den = max_i |e_i| / max(|y_i|, |ynew_i|, thr) */
 };
 
 /* keeps the larger of two ratios na/da, nb/db (all >= 0, denominators > 0) by cross-multiplication */
@@ -175,94 +258,145 @@ IA_DEV void ia_ratio_max(double &na, double &da, double nb, double db) {
     da = gt ? db : da;
 }
 
-/* One uncontrolled DP5(4) step of size h from (tf, x, v) with A1 = A(tf, x) given.
- * Out: xn, vn (5th-order solution), A7 = A(tf + h, xn) (FSAL), r2n = |d(xn)|^2, the error-norm
- * argmax pair, and finite = false when the step produced a non-finite separation. */
-IA_DEV void ia_dp5_attempt(const IaParams &P, const double (&x)[6], const double (&v)[6], const double (&A1)[6],
-                           double tf, double phase, double h, double (&xn)[6], double (&vn)[6],
-                           double (&A7)[6], double &r2n, IaErr &err, bool &finite) {
+/* per-lane trajectory state: positions, velocities and the FSAL acceleration of the local axes */
+template <int LPT>
+struct IaVec {
+    static constexpr int NA = 3 / LPT;
+    double xi[NA], xa[NA], vi[NA], va[NA], Ai[NA], Aa[NA];
+};
+
+/* what one attempt returns besides the new state */
+struct IaStepOut {
+    IaErr err;    /* error-norm argmax pair                                   */
+    double r2n;   /* |d|^2 at the new state                                   */
+    double s_new; /* d.w at the new state (sign of dr/dt, reading R6)         */
+    bool finite;  /* false when the step produced a non-finite separation     */
+};
+
+/* One uncontrolled DP5(4) step of size h from state Y (with Y.A = A(tf, x), FSAL) to N (with N.A =
+ * A(tf + h, x_new)).  Every lane of the warp must call this together when LPT = 3. */
+template <int LPT, bool FUSED>
+IA_DEV void ia_dp5_attempt(const IaParams &P, const IaLane<LPT> &L, const IaVec<LPT> &Y, double tf, double phase,
+                           double h, IaVec<LPT> &N, IaStepOut &out) {
+    constexpr int NA = 3 / LPT;
     const double hh = h * h;
-    double X[6], A2[6], A3[6], A4[6], A5[6], A6[6];
-    double r2, s;
+    /* the stage cosines depend on (tf, h) only: independent chains that fill the latency of the serial
+     * r^2 -> 1/r^2 -> force chain; each is released two stages ahead of its use */
+    const double hc2 = h * IA_C2, hc3 = h * IA_C3, hc4 = h * IA_C4, hc5 = h * IA_C5;
+    const double cs2 = ia_cos_folded(ia_fma<FUSED>(P.omega, tf + hc2, phase));
+    const double cs3 = ia_cos_folded(ia_fma<FUSED>(P.omega, tf + hc3, phase));
+    double Xi[NA], Xa[NA], D[3], r2, s;
+    double A2i[NA], A2a[NA], A3i[NA], A3a[NA], A4i[NA], A4a[NA], A5i[NA], A5a[NA], A6i[NA], A6a[NA];
+#define IA_F(a, b, c) ia_fma<FUSED>(a, b, c)
     /* stage 2 */
-    {
-        const double hc = h * IA_C2;
 #pragma unroll
-        for (int i = 0; i < 6; ++i) X[i] = x[i] + hc * v[i];
-        const double c = ia_cos_folded(P.omega * (tf + hc) + phase);
-        ia_accel(P, X, c, A2, r2, s);
+    for (int a = 0; a < NA; ++a) {
+        Xi[a] = IA_F(hc2, Y.vi[a], Y.xi[a]);
+        Xa[a] = IA_F(hc2, Y.va[a], Y.xa[a]);
     }
+    ia_accel<LPT, FUSED>(P, L, Xi, Xa, cs2, A2i, A2a, D, r2, s);
+    double t4 = tf + hc4;
+    IA_TIE(t4, A2a[0]);
+    const double cs4 = ia_cos_folded(ia_fma<FUSED>(P.omega, t4, phase));
     /* stage 3 */
     {
-        const double hc = h * IA_C3, g1 = hh * IA_AB31;
+        const double g1 = hh * IA_AB31;
 #pragma unroll
-        for (int i = 0; i < 6; ++i) X[i] = x[i] + hc * v[i] + g1 * A1[i];
-        const double c = ia_cos_folded(P.omega * (tf + hc) + phase);
-        ia_accel(P, X, c, A3, r2, s);
+        for (int a = 0; a < NA; ++a) {
+            Xi[a] = IA_F(g1, Y.Ai[a], IA_F(hc3, Y.vi[a], Y.xi[a]));
+            Xa[a] = IA_F(g1, Y.Aa[a], IA_F(hc3, Y.va[a], Y.xa[a]));
+        }
+        ia_accel<LPT, FUSED>(P, L, Xi, Xa, cs3, A3i, A3a, D, r2, s);
     }
+    double t5 = tf + hc5;
+    IA_TIE(t5, A3a[0]);
+    const double cs5 = ia_cos_folded(ia_fma<FUSED>(P.omega, t5, phase));
     /* stage 4 */
     {
-        const double hc = h * IA_C4, g1 = hh * IA_AB41, g2 = hh * IA_AB42;
+        const double g1 = hh * IA_AB41, g2 = hh * IA_AB42;
 #pragma unroll
-        for (int i = 0; i < 6; ++i) X[i] = x[i] + hc * v[i] + g1 * A1[i] + g2 * A2[i];
-        const double c = ia_cos_folded(P.omega * (tf + hc) + phase);
-        ia_accel(P, X, c, A4, r2, s);
+        for (int a = 0; a < NA; ++a) {
+            Xi[a] = IA_F(g2, A2i[a], IA_F(g1, Y.Ai[a], IA_F(hc4, Y.vi[a], Y.xi[a])));
+            Xa[a] = IA_F(g2, A2a[a], IA_F(g1, Y.Aa[a], IA_F(hc4, Y.va[a], Y.xa[a])));
+        }
+        ia_accel<LPT, FUSED>(P, L, Xi, Xa, cs4, A4i, A4a, D, r2, s);
     }
+    double t1 = tf + h; /* stages 6 and 7 share the time t + h */
+    IA_TIE(t1, A4a[0]);
+    const double cs1 = ia_cos_folded(ia_fma<FUSED>(P.omega, t1, phase));
     /* stage 5 */
     {
-        const double hc = h * IA_C5, g1 = hh * IA_AB51, g2 = hh * IA_AB52, g3 = hh * IA_AB53;
+        const double g1 = hh * IA_AB51, g2 = hh * IA_AB52, g3 = hh * IA_AB53;
 #pragma unroll
-        for (int i = 0; i < 6; ++i) X[i] = x[i] + hc * v[i] + g1 * A1[i] + g2 * A2[i] + g3 * A3[i];
-        const double c = ia_cos_folded(P.omega * (tf + hc) + phase);
-        ia_accel(P, X, c, A5, r2, s);
+        for (int a = 0; a < NA; ++a) {
+            Xi[a] = IA_F(g3, A3i[a], IA_F(g2, A2i[a], IA_F(g1, Y.Ai[a], IA_F(hc5, Y.vi[a], Y.xi[a]))));
+            Xa[a] = IA_F(g3, A3a[a], IA_F(g2, A2a[a], IA_F(g1, Y.Aa[a], IA_F(hc5, Y.va[a], Y.xa[a]))));
+        }
+        ia_accel<LPT, FUSED>(P, L, Xi, Xa, cs5, A5i, A5a, D, r2, s);
     }
-    /* stages 6 and 7 share the time t + h, hence the cosine */
-    const double c1 = ia_cos_folded(P.omega * (tf + h) + phase);
+    /* stage 6 */
     {
         const double g1 = hh * IA_AB61, g2 = hh * IA_AB62, g3 = hh * IA_AB63, g4 = hh * IA_AB64;
 #pragma unroll
-        for (int i = 0; i < 6; ++i) X[i] = x[i] + h * v[i] + g1 * A1[i] + g2 * A2[i] + g3 * A3[i] + g4 * A4[i];
-        ia_accel(P, X, c1, A6, r2, s);
+        for (int a = 0; a < NA; ++a) {
+            Xi[a] = IA_F(g4, A4i[a], IA_F(g3, A3i[a], IA_F(g2, A2i[a], IA_F(g1, Y.Ai[a], IA_F(h, Y.vi[a], Y.xi[a])))));
+            Xa[a] = IA_F(g4, A4a[a], IA_F(g3, A3a[a], IA_F(g2, A2a[a], IA_F(g1, Y.Aa[a], IA_F(h, Y.va[a], Y.xa[a])))));
+        }
+        ia_accel<LPT, FUSED>(P, L, Xi, Xa, cs1, A6i, A6a, D, r2, s);
     }
-    /* 5th-order solution: x_new = X_7, v_new = v + h sum b_l A_l */
+    /* 5th-order solution x_new = X_7, v_new = v + h sum b_l A_l, and the error sums over stages 1..6,
+     * component by component so that A3..A6 die here; stage 7 = FSAL adds its term afterwards */
+    double exi[NA], exa[NA], evi[NA], eva[NA];
     {
         const double g1 = hh * IA_AB71, g3 = hh * IA_AB73, g4 = hh * IA_AB74, g5 = hh * IA_AB75;
         const double w1 = h * IA_B1, w3 = h * IA_B3, w4 = h * IA_B4, w5 = h * IA_B5, w6 = h * IA_B6;
-#pragma unroll
-        for (int i = 0; i < 6; ++i) {
-            xn[i] = x[i] + h * v[i] + g1 * A1[i] + g3 * A3[i] + g4 * A4[i] + g5 * A5[i];
-            vn[i] = v[i] + w1 * A1[i] + w3 * A3[i] + w4 * A4[i] + w5 * A5[i] + w6 * A6[i];
-        }
-        ia_accel(P, xn, c1, A7, r2n, s);
-    }
-    finite = (s == s); /* s is NaN whenever r2 of stage 7 is 0, inf or NaN (see ia_rcp) */
-    /* error estimate and ode45 norm (R5) */
-    {
         const double q1 = hh * IA_EB1, q3 = hh * IA_EB3, q4 = hh * IA_EB4, q5 = hh * IA_EB5, q6 = hh * IA_EB6;
-        const double p1 = h * IA_E1, p3 = h * IA_E3, p4 = h * IA_E4, p5 = h * IA_E5, p6 = h * IA_E6, p7 = h * IA_E7;
-        double en[12], sc[12];
+        const double p1 = h * IA_E1, p3 = h * IA_E3, p4 = h * IA_E4, p5 = h * IA_E5, p6 = h * IA_E6;
 #pragma unroll
-        for (int i = 0; i < 6; ++i) {
-            const double ex = q1 * A1[i] + q3 * A3[i] + q4 * A4[i] + q5 * A5[i] + q6 * A6[i];
-            const double ev = p1 * A1[i] + p3 * A3[i] + p4 * A4[i] + p5 * A5[i] + p6 * A6[i] + p7 * A7[i];
-            en[i] = fabs(ex);
-            en[6 + i] = fabs(ev);
-            sc[i] = fmax(fmax(fabs(x[i]), fabs(xn[i])), P.thr);
-            sc[6 + i] = fmax(fmax(fabs(v[i]), fabs(vn[i])), P.thr);
+        for (int a = 0; a < NA; ++a) {
+            N.xi[a] = IA_F(g5, A5i[a], IA_F(g4, A4i[a], IA_F(g3, A3i[a], IA_F(g1, Y.Ai[a], IA_F(h, Y.vi[a], Y.xi[a])))));
+            N.vi[a] = IA_F(w6, A6i[a], IA_F(w5, A5i[a], IA_F(w4, A4i[a], IA_F(w3, A3i[a], IA_F(w1, Y.Ai[a], Y.vi[a])))));
+            exi[a] = IA_F(q6, A6i[a], IA_F(q5, A5i[a], IA_F(q4, A4i[a], IA_F(q3, A3i[a], q1 * Y.Ai[a]))));
+            evi[a] = IA_F(p6, A6i[a], IA_F(p5, A5i[a], IA_F(p4, A4i[a], IA_F(p3, A3i[a], p1 * Y.Ai[a]))));
+            N.xa[a] = IA_F(g5, A5a[a], IA_F(g4, A4a[a], IA_F(g3, A3a[a], IA_F(g1, Y.Aa[a], IA_F(h, Y.va[a], Y.xa[a])))));
+            N.va[a] = IA_F(w6, A6a[a], IA_F(w5, A5a[a], IA_F(w4, A4a[a], IA_F(w3, A3a[a], IA_F(w1, Y.Aa[a], Y.va[a])))));
+            exa[a] = IA_F(q6, A6a[a], IA_F(q5, A5a[a], IA_F(q4, A4a[a], IA_F(q3, A3a[a], q1 * Y.Aa[a]))));
+            eva[a] = IA_F(p6, A6a[a], IA_F(p5, A5a[a], IA_F(p4, A4a[a], IA_F(p3, A3a[a], p1 * Y.Aa[a]))));
         }
-        /* tree of cross-multiplied comparisons */
-#pragma unroll
-        for (int i = 0; i < 6; ++i) ia_ratio_max(en[i], sc[i], en[6 + i], sc[6 + i]);
-#pragma unroll
-        for (int i = 0; i < 3; ++i) ia_ratio_max(en[i], sc[i], en[3 + i], sc[3 + i]);
-        ia_ratio_max(en[0], sc[0], en[1], sc[1]);
-        ia_ratio_max(en[0], sc[0], en[2], sc[2]);
-        err.num = en[0];
-        err.den = sc[0];
+        ia_accel<LPT, FUSED>(P, L, N.xi, N.xa, cs1, N.Ai, N.Aa, D, out.r2n, s);
     }
-}
-
-/* d.w with d = r_a - r_i, w = v_a - v_i: sign of dr/dt (reading R6) */
-IA_DEV double ia_sdot(const double (&x)[6], const double (&v)[6]) {
-    return (x[3] - x[0]) * (v[3] - v[0]) + (x[4] - x[1]) * (v[4] - v[1]) + (x[5] - x[2]) * (v[5] - v[2]);
+    out.finite = (s == s); /* s is NaN whenever r2 of stage 7 is 0, inf or NaN (see ia_rcp) */
+    /* d.w at the new state */
+    {
+        double w[NA], W[3];
+#pragma unroll
+        for (int a = 0; a < NA; ++a) w[a] = N.va[a] - N.vi[a];
+        ia_gather3<LPT>(L, w, W);
+        out.s_new = ia_dot3<FUSED>(D, W);
+    }
+    /* ode45 norm (R5): per axis the tree (x_i vs v_i), (x_a vs v_a), (ion vs atom); then axis 0 vs 1, then vs 2 */
+    {
+        const double p7 = h * IA_E7;
+        double en[NA], sc[NA];
+#pragma unroll
+        for (int a = 0; a < NA; ++a) {
+            const double fvi = IA_F(p7, N.Ai[a], evi[a]);
+            const double fva = IA_F(p7, N.Aa[a], eva[a]);
+            double n_i = fabs(exi[a]), d_i = fmax(fmax(fabs(Y.xi[a]), fabs(N.xi[a])), P.thr);
+            ia_ratio_max(n_i, d_i, fabs(fvi), fmax(fmax(fabs(Y.vi[a]), fabs(N.vi[a])), P.thr));
+            double n_a = fabs(exa[a]), d_a = fmax(fmax(fabs(Y.xa[a]), fabs(N.xa[a])), P.thr);
+            ia_ratio_max(n_a, d_a, fabs(fva), fmax(fmax(fabs(Y.va[a]), fabs(N.va[a])), P.thr));
+            ia_ratio_max(n_i, d_i, n_a, d_a);
+            en[a] = n_i;
+            sc[a] = d_i;
+        }
+        double EN[3], SC[3];
+        ia_gather3<LPT>(L, en, EN);
+        ia_gather3<LPT>(L, sc, SC);
+        ia_ratio_max(EN[0], SC[0], EN[1], SC[1]);
+        ia_ratio_max(EN[0], SC[0], EN[2], SC[2]);
+        out.err.num = EN[0];
+        out.err.den = SC[0];
+    }
+#undef IA_F
 }

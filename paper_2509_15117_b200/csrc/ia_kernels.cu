@@ -1,20 +1,26 @@
 /*
- * ia_kernels.cu -- the persistent propagation kernel (K1), the initial-condition generator (K2)
- * and the production-arithmetic build of the verification kernels (K3).
+ * ia_kernels.cu -- the persistent propagation kernels (K1 bulk, K5 straggler), the initial-condition
+ * generator (K2) and the verification kernels (K3).  Compiled with -fmad=false: see ia_dev.cuh.
  *
- * K1: one lane = one trajectory.  State, accelerations of all seven stages, step size and event
- * bookkeeping live in registers; nothing per step touches memory.  A lane whose trajectory has
- * terminated writes its 64-byte record, adds to the ensemble summary and takes the next index from
- * a global work counter (one atomicAdd per warp-refill), so warps stay full although trajectory
- * lengths span 10^3..10^7 steps.
- * Exit localisation (reading R7) re-uses the same step body with the lane in mode LOC, so the warp
- * never diverges on it.
+ * ia_persistent_kernel<LPT>: state, accelerations of all seven stages, step size and event
+ * bookkeeping live in registers; nothing per step touches memory.  A group of LPT lanes owns one
+ * trajectory.  A group whose trajectory has terminated writes its 64-byte record, adds to the
+ * ensemble summary and takes the next index from a global work counter (one atomicAdd per
+ * warp-refill), so warps stay full although trajectory lengths span 10^3..10^7 steps
+ * (DESIGN.md "Persistent loop").  Exit localisation (reading R7) re-uses the same
+ * step body with the group in mode LOC, so the warp never diverges on it.
+ *
+ *   K1 = <1>: one lane per trajectory, the throughput layout.  Once the work counter is empty and a
+ *        warp is down to `handoff_lanes` running lanes it writes their states to a queue and exits.
+ *   K5 = <3>: three lanes per trajectory (x/y/z split), launched behind K1 on the same stream; it
+ *        resumes the queued stragglers.  A third of the FP64 instructions per lane and step: what
+ *        counts for the last, longest trajectories is the latency of one step, not throughput.
+ * Both run the same arithmetic (ia_dev.cuh) and give bit-identical trajectories, so where a
+ * trajectory is handed over does not show in its result.
  */
 #include "ia_kernels.cuh"
 
-#define IA_WARPS_PER_BLOCK 1
-#define IA_THREADS (32 * IA_WARPS_PER_BLOCK)
-#define IA_FULL 0xffffffffu
+#define IA_THREADS 32
 
 enum { MODE_IDLE = 0, MODE_RUN = 1, MODE_LOC = 2 };
 
@@ -40,17 +46,23 @@ __device__ __forceinline__ double ia_u53(unsigned we, unsigned wo) {
     return ((double)(we >> 5) * 67108864.0 + (double)(wo >> 6) + 0.5) * (1.0 / 9007199254740992.0);
 }
 
-/* Initial condition of local trajectory j: x = (r_i, r_a), v = (v_i, v_a), rf phase, energy. */
-__device__ __noinline__ void ia_generate_ic(const IaParams &P, const IaGen &G, unsigned long long j, double (&x)[6],
-                                            double (&v)[6], double &phase, double &E_au) {
+struct IaIC {
+    double x[6], v[6]; /* r_i, r_a | v_i, v_a */
+    double phase, E_au;
+};
+
+/* Initial condition of local trajectory j.  Out of line and writing through a pointer on purpose:
+ * the struct lives in the stack frame for the duration of a refill only, and the persistent state
+ * of the caller stays in registers. */
+__device__ __forceinline__ void ia_generate_ic(const IaParams &P, const IaGen &G, unsigned long long j, IaIC *ic) {
     if (G.mode == IA_IC_EXPLICIT) {
 #pragma unroll
         for (int i = 0; i < 6; ++i) {
-            x[i] = G.y0[j * 12 + i];
-            v[i] = G.y0[j * 12 + 6 + i];
+            ic->x[i] = G.y0[j * 12 + i];
+            ic->v[i] = G.y0[j * 12 + 6 + i];
         }
-        phase = G.phase[j];
-        E_au = 0.5 * P.m_a * (v[3] * v[3] + v[4] * v[4] + v[5] * v[5]);
+        ic->phase = G.phase[j];
+        ic->E_au = 0.5 * P.m_a * (ic->v[3] * ic->v[3] + ic->v[4] * ic->v[4] + ic->v[5] * ic->v[5]);
         return;
     }
     const unsigned long long gi = G.first_index + j;
@@ -70,39 +82,40 @@ __device__ __noinline__ void ia_generate_ic(const IaParams &P, const IaGen &G, u
         st = sqrt(1.0 - ct * ct);
         sincospi(G.phi_span_pi * u2, &sp, &cp);
     }
-    phase = (G.phase_mode == 1) ? 6.28318530717958647692 * u3 : G.phase0;
+    ic->phase = (G.phase_mode == 1) ? 6.28318530717958647692 * u3 : G.phase0;
     double v0;
     if (G.log_E_ratio != 0.0) {
         const double E_uK = G.E_min_uK * exp(u4 * G.log_E_ratio);
-        E_au = E_uK * 1e-6 * 3.1668115634564e-6; /* k_B in E_h/K (CODATA 2022) */
-        v0 = sqrt(2.0 * E_au / P.m_a);
+        ic->E_au = E_uK * 1e-6 * 3.1668115634564e-6; /* k_B in E_h/K (CODATA 2022) */
+        v0 = sqrt(2.0 * ic->E_au / P.m_a);
     } else {
-        E_au = G.E_fixed_au;
+        ic->E_au = G.E_fixed_au;
         v0 = G.v0_fixed;
     }
     const double n0 = st * cp, n1 = st * sp, n2 = ct;
-    x[0] = 0.0; x[1] = 0.0; x[2] = 0.0;           /* ion at the trap centre, at rest */
-    v[0] = 0.0; v[1] = 0.0; v[2] = 0.0;
-    x[3] = P.r0 * n0; x[4] = P.r0 * n1; x[5] = P.r0 * n2;   /* atom on the r0 sphere ...            */
-    v[3] = -v0 * n0; v[4] = -v0 * n1; v[5] = -v0 * n2;      /* ... aimed at the ion                */
+    ic->x[0] = 0.0; ic->x[1] = 0.0; ic->x[2] = 0.0;   /* ion at the trap centre, at rest */
+    ic->v[0] = 0.0; ic->v[1] = 0.0; ic->v[2] = 0.0;
+    ic->x[3] = P.r0 * n0; ic->x[4] = P.r0 * n1; ic->x[5] = P.r0 * n2;   /* atom on the r0 sphere ...   */
+    ic->v[3] = -v0 * n0; ic->v[4] = -v0 * n1; ic->v[5] = -v0 * n2;      /* ... aimed at the ion        */
 }
 
-__global__ void ia_generate_kernel(IaParams P, IaGen G, double *ic_dump) {
+__global__ void ia_generate_kernel(const __grid_constant__ IaParams P, const __grid_constant__ IaGen G,
+                                   double *ic_dump) {
     const unsigned long long j = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= G.n) return;
-    double x[6], v[6], phase, E;
-    ia_generate_ic(P, G, j, x, v, phase, E);
+    IaIC ic;
+    ia_generate_ic(P, G, j, &ic);
     double *o = ic_dump + j * 14;
 #pragma unroll
     for (int i = 0; i < 6; ++i) {
-        o[i] = x[i];
-        o[6 + i] = v[i];
+        o[i] = ic.x[i];
+        o[6 + i] = ic.v[i];
     }
-    o[12] = phase;
-    o[13] = E;
+    o[12] = ic.phase;
+    o[13] = ic.E_au;
 }
 
-/* ---- per-trajectory set-up (reading R5: ode45 initial step) --------------------------------- */
+/* ---- helpers ---------------------------------------------------------------------------------- */
 
 __device__ __forceinline__ bool ia_isfinite(double a) { return fabs(a) <= 1.79769313486231570815e308; }
 
@@ -112,273 +125,456 @@ __device__ __forceinline__ unsigned long long ia_globaltimer() {
     return t;
 }
 
-/* ---- K1 ------------------------------------------------------------------------------------- */
+/* element `axis` (0..2) of a 3-array held in registers, without dynamic indexing */
+__device__ __forceinline__ double ia_sel3(double a0, double a1, double a2, unsigned axis) {
+    return axis == 0u ? a0 : (axis == 1u ? a1 : a2);
+}
 
-__global__ void __launch_bounds__(IA_THREADS) ia_persistent_kernel(const __grid_constant__ IaParams P,
-                                                                  const __grid_constant__ IaGen G, IaOut O,
-                                                                  unsigned long long *counter,
-                                                                  unsigned long long warn) {
-    const unsigned lane = threadIdx.x & 31u;
-    /* lane state */
-    double x[6], v[6], A1[6];
-    double tf = 0.0, h = 0.0, phase = 0.0, s_old = 0.0, t_first = 0.0, t_last = 0.0;
-    unsigned n_per = 0, n_coll = 0, n_tp = 0, steps_acc = 0, steps_rej = 0, n_loc = 0;
-    unsigned long long slot = 0;
-    int mode = MODE_IDLE;
-    bool failed = false, exhausted = false;
+template <int LPT>
+__device__ __forceinline__ void ia_park(const IaLane<LPT> &L, IaVec<LPT> &Y) {
+    /* harmless finite state for idle lanes: ion at the origin, atom at (4,5,6) */
 #pragma unroll
-    for (int i = 0; i < 6; ++i) {
-        x[i] = (i < 3) ? 0.0 : 1.0 + i; /* harmless finite state for idle lanes */
-        v[i] = 0.0;
-        A1[i] = 0.0;
+    for (int a = 0; a < 3 / LPT; ++a) {
+        Y.xi[a] = 0.0;
+        Y.xa[a] = 4.0 + (double)(L.axis0 + a);
+        Y.vi[a] = 0.0; Y.va[a] = 0.0; Y.Ai[a] = 0.0; Y.Aa[a] = 0.0;
     }
-    if (O.summary != nullptr && threadIdx.x == 0) {
+}
+
+/* ---- K1 / K5 ---------------------------------------------------------------------------------- */
+
+template <int LPT>
+__global__ void __launch_bounds__(IA_THREADS, LPT == 1 ? 12 : 16)
+ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__ IaGen G, const IaOut O,
+                     const IaSched S) {
+    constexpr int NA = 3 / LPT;
+    const unsigned lane = threadIdx.x & 31u;
+    const IaLane<LPT> L = ia_make_lane<LPT>(P, lane);
+    /* group state (replicated in the LPT lanes of a group) */
+    IaVec<LPT> Y;
+    double tf = 0.0, h = 0.0;
+    unsigned n_per = 0, steps_acc = 0;
+    /* rarely touched per-group state lives in shared memory, not in registers */
+    __shared__ double sh_t_first[IA_THREADS], sh_t_last[IA_THREADS], sh_phase[IA_THREADS], sh_s_old[IA_THREADS];
+    __shared__ unsigned long long sh_slot[IA_THREADS];
+    __shared__ unsigned sh_steps_in[IA_THREADS], sh_n_coll[IA_THREADS], sh_n_tp[IA_THREADS], sh_n_loc[IA_THREADS],
+        sh_steps_rej[IA_THREADS];
+    double &t_first = sh_t_first[threadIdx.x], &t_last = sh_t_last[threadIdx.x], &phase = sh_phase[threadIdx.x],
+           &s_old = sh_s_old[threadIdx.x];
+    phase = 0.0; s_old = 0.0;
+    unsigned long long &slot = sh_slot[threadIdx.x];
+    unsigned &steps_in = sh_steps_in[threadIdx.x], &n_coll = sh_n_coll[threadIdx.x], &n_tp = sh_n_tp[threadIdx.x],
+             &n_loc = sh_n_loc[threadIdx.x], &steps_rej = sh_steps_rej[threadIdx.x];
+    t_first = 0.0; t_last = 0.0; slot = 0; steps_in = 0; n_coll = 0; n_tp = 0; n_loc = 0; steps_rej = 0;
+    int mode = MODE_IDLE;
+    bool failed = false;
+    bool wexh = false; /* warp-uniform: the work counter is empty */
+    ia_park<LPT>(L, Y);
+    if (O.summary != nullptr && threadIdx.x == 0 && S.q_in == nullptr) {
         const unsigned long long t0 = ia_globaltimer();
         if (blockIdx.x == 0) {
             atomicCAS((unsigned long long *)&O.summary->t_start_ns, 0ull, t0);
-            if (warn) atomicOr((unsigned long long *)&O.summary->warn, warn);
+            if (S.warn) atomicOr((unsigned long long *)&O.summary->warn, S.warn);
         }
     }
 
     for (;;) {
-        /* ---- refill idle lanes from the global work counter (a12) ---- */
-        const bool want = (mode == MODE_IDLE) && !exhausted;
-        const unsigned wm = __ballot_sync(IA_FULL, want);
+        /* ---- refill idle groups from the global work counter (a12) ---- */
+        const bool want = L.valid && (mode == MODE_IDLE) && !wexh;
+        const unsigned wm = __ballot_sync(IA_FULL, want && L.leader);
         if (wm) {
-            const int leader = __ffs(wm) - 1;
+            const int first = __ffs(wm) - 1;
             unsigned long long base = 0;
-            if ((int)lane == leader) base = atomicAdd(counter, (unsigned long long)__popc(wm));
-            base = __shfl_sync(IA_FULL, base, leader);
-            if (want) {
-                const unsigned long long j = base + __popc(wm & ((1u << lane) - 1u));
-                if (j >= G.n) {
-                    exhausted = true;
-                    if (O.summary != nullptr)
-                        atomicCAS((unsigned long long *)&O.summary->t_first_idle_ns, 0ull, ia_globaltimer());
+            if ((int)lane == first) base = atomicAdd(S.counter, (unsigned long long)__popc(wm));
+            base = __shfl_sync(IA_FULL, base, first);
+            const unsigned long long j = base + __popc(wm & ((1u << L.gbase) - 1u));
+            const unsigned long long n_total = (S.q_in != nullptr) ? *S.n_in : G.n;
+            const bool got = want && (j < n_total);
+            if (__any_sync(IA_FULL, want && !got)) {
+                if (!wexh && O.summary != nullptr && S.q_in == nullptr && lane == 0)
+                    atomicCAS((unsigned long long *)&O.summary->t_first_idle_ns, 0ull, ia_globaltimer());
+                wexh = true;
+            }
+            if (got) {
+                if (S.q_in != nullptr) {
+                    /* resume a trajectory the bulk kernel handed over */
+                    const IaHand *H = S.q_in + j;
+#pragma unroll
+                    for (int a = 0; a < NA; ++a) {
+                        const unsigned ax = L.axis0 + a;
+                        Y.xi[a] = H->x[ax];  Y.xa[a] = H->x[3 + ax];
+                        Y.vi[a] = H->v[ax];  Y.va[a] = H->v[3 + ax];
+                        Y.Ai[a] = H->A1[ax]; Y.Aa[a] = H->A1[3 + ax];
+                    }
+                    tf = H->tf; h = H->h; phase = H->phase; s_old = H->s_old;
+                    t_first = H->t_first; t_last = H->t_last; slot = H->slot;
+                    n_per = H->n_per; n_coll = H->n_coll; n_tp = H->n_tp;
+                    steps_acc = H->steps_acc; steps_rej = H->steps_rej; failed = H->failed != 0u;
+                    steps_in = steps_acc + steps_rej;
+                    n_loc = 0;
+                    mode = MODE_RUN;
                 } else {
-                    double E_au;
-                    ia_generate_ic(P, G, j, x, v, phase, E_au);
-                    if (O.ic_dump != nullptr) {
+                    IaIC ic;
+                    ia_generate_ic(P, G, j, &ic);
+                    if (O.ic_dump != nullptr && L.leader) {
                         double *o = O.ic_dump + j * 14;
 #pragma unroll
                         for (int i = 0; i < 6; ++i) {
-                            o[i] = x[i];
-                            o[6 + i] = v[i];
+                            o[i] = ic.x[i];
+                            o[6 + i] = ic.v[i];
                         }
-                        o[12] = phase;
-                        o[13] = E_au;
+                        o[12] = ic.phase;
+                        o[13] = ic.E_au;
                     }
                     slot = j;
-                    tf = 0.0; n_per = 0; n_coll = 0; n_tp = 0; steps_acc = 0; steps_rej = 0; n_loc = 0;
+                    tf = 0.0; n_per = 0; n_coll = 0; n_tp = 0; steps_acc = 0; steps_rej = 0; n_loc = 0; steps_in = 0;
                     t_first = 0.0; t_last = 0.0; failed = false;
+                    phase = ic.phase;
                     bool ok = ia_isfinite(phase);
 #pragma unroll
-                    for (int i = 0; i < 6; ++i) ok = ok && ia_isfinite(x[i]) && ia_isfinite(v[i]);
+                    for (int i = 0; i < 6; ++i) ok = ok && ia_isfinite(ic.x[i]) && ia_isfinite(ic.v[i]);
                     if (!ok) {
                         /* status 3: non-finite initial state; record it and stay idle */
-                        if (O.records != nullptr) {
-                            ia_record r;
-                            r.ke_ion = 0.5 * P.m_i * (v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
-                            r.t_dwell = 0.0; r.t_life = 0.0;
-                            r.va_f[0] = v[3]; r.va_f[1] = v[4]; r.va_f[2] = v[5];
-                            r.n_coll = 0; r.n_tp = 0; r.steps_acc = 0; r.steps_rej = 0; r.status = 3; r.n_loc = 0;
-                            O.records[j] = r;
-                        }
-                        if (O.summary != nullptr) {
-                            atomicAdd((unsigned long long *)&O.summary->n_done, 1ull);
-                            atomicAdd((unsigned long long *)&O.summary->n_status[3], 1ull);
-                            atomicAdd((unsigned long long *)&O.summary->hist_ncoll[0], 1ull);
-                        }
-#pragma unroll
-                        for (int i = 0; i < 6; ++i) {
-                            x[i] = (i < 3) ? 0.0 : 1.0 + i;
-                            v[i] = 0.0;
+                        if (L.leader) {
+                            if (O.records != nullptr) {
+                                ia_record r;
+                                r.ke_ion = 0.5 * P.m_i * (ic.v[0] * ic.v[0] + ic.v[1] * ic.v[1] + ic.v[2] * ic.v[2]);
+                                r.t_dwell = 0.0; r.t_life = 0.0;
+                                r.va_f[0] = ic.v[3]; r.va_f[1] = ic.v[4]; r.va_f[2] = ic.v[5];
+                                r.n_coll = 0; r.n_tp = 0; r.steps_acc = 0; r.steps_rej = 0; r.status = 3; r.n_loc = 0;
+                                O.records[j] = r;
+                            }
+                            if (O.summary != nullptr) {
+                                atomicAdd((unsigned long long *)&O.summary->n_done, 1ull);
+                                atomicAdd((unsigned long long *)&O.summary->n_status[3], 1ull);
+                                atomicAdd((unsigned long long *)&O.summary->hist_ncoll[0], 1ull);
+                            }
                         }
                         phase = 0.0;
                     } else {
                         /* keep the cosine argument in the folded range for any caller-supplied phase */
                         if (fabs(phase) > 6.5) phase -= 6.28318530717958647692 * rint(phase * 0.15915494309189533577);
-                        double r2, s;
-                        ia_accel(P, x, ia_cos_folded(phase), A1, r2, s);
-                        /* h = min(h_max, t_max); rho = ||f0 / max(|y0|, thr)||_inf / (0.8 rtol^(1/5)) */
+                        /* A(0, x0) for all six components in the one-lane layout (same arithmetic per
+                         * component as the group layout), then the ode45 first step (R5):
+                         * h = min(h_max, t_max); rho = ||f0 / max(|y0|, thr)||_inf / (0.8 rtol^(1/5)) */
+                        const IaLane<1> L1 = ia_make_lane<1>(P, lane);
+                        const double xi3[3] = {ic.x[0], ic.x[1], ic.x[2]}, xa3[3] = {ic.x[3], ic.x[4], ic.x[5]};
+                        double ai3[3], aa3[3], D[3], r2, s;
+                        ia_accel<1, true>(P, L1, xi3, xa3, ia_cos_folded(phase), ai3, aa3, D, r2, s);
                         double rho = 0.0;
 #pragma unroll
-                        for (int i = 0; i < 6; ++i) {
-                            rho = fmax(rho, fabs(v[i]) / fmax(fabs(x[i]), P.thr));
-                            rho = fmax(rho, fabs(A1[i]) / fmax(fabs(v[i]), P.thr));
+                        for (int i = 0; i < 3; ++i) {
+                            rho = fmax(rho, fabs(ic.v[i]) / fmax(fabs(ic.x[i]), P.thr));
+                            rho = fmax(rho, fabs(ic.v[3 + i]) / fmax(fabs(ic.x[3 + i]), P.thr));
+                            rho = fmax(rho, fabs(ai3[i]) / fmax(fabs(ic.v[i]), P.thr));
+                            rho = fmax(rho, fabs(aa3[i]) / fmax(fabs(ic.v[3 + i]), P.thr));
                         }
                         rho = rho / P.h0_scale;
                         h = fmin(P.h_max, P.t_max);
                         if (h * rho > 1.0) h = 1.0 / rho;
                         if (h < P.h_min) h = P.h_min;
-                        s_old = ia_sdot(x, v);
+                        const double W[3] = {ic.v[3] - ic.v[0], ic.v[4] - ic.v[1], ic.v[5] - ic.v[2]};
+                        s_old = ia_dot3<true>(D, W);
+#pragma unroll
+                        for (int a = 0; a < NA; ++a) {
+                            const unsigned ax = L.axis0 + a;
+                            Y.xi[a] = (LPT == 1) ? ic.x[a] : ia_sel3(ic.x[0], ic.x[1], ic.x[2], ax);
+                            Y.xa[a] = (LPT == 1) ? ic.x[3 + a] : ia_sel3(ic.x[3], ic.x[4], ic.x[5], ax);
+                            Y.vi[a] = (LPT == 1) ? ic.v[a] : ia_sel3(ic.v[0], ic.v[1], ic.v[2], ax);
+                            Y.va[a] = (LPT == 1) ? ic.v[3 + a] : ia_sel3(ic.v[3], ic.v[4], ic.v[5], ax);
+                            Y.Ai[a] = (LPT == 1) ? ai3[a] : ia_sel3(ai3[0], ai3[1], ai3[2], ax);
+                            Y.Aa[a] = (LPT == 1) ? aa3[a] : ia_sel3(aa3[0], aa3[1], aa3[2], ax);
+                        }
                         mode = MODE_RUN;
                     }
                 }
             }
         }
+
+        /* ---- hand the last running lanes of a drained warp over to the straggler kernel ---- */
+        if (LPT == 1 && S.q_out != nullptr && wexh) {
+            const unsigned am = __ballot_sync(IA_FULL, mode == MODE_RUN);
+            const unsigned lm = __ballot_sync(IA_FULL, mode == MODE_LOC);
+            if (am != 0u && lm == 0u && __popc(am) <= S.handoff_lanes) {
+                const int first = __ffs(am) - 1;
+                unsigned long long base = 0;
+                if ((int)lane == first) base = atomicAdd(S.n_out, (unsigned long long)__popc(am));
+                base = __shfl_sync(IA_FULL, base, first);
+                if (mode == MODE_RUN) {
+                    IaHand *H = S.q_out + base + __popc(am & ((1u << lane) - 1u));
+#pragma unroll
+                    for (int a = 0; a < NA; ++a) {
+                        H->x[a] = Y.xi[a];  H->x[3 + a] = Y.xa[a];
+                        H->v[a] = Y.vi[a];  H->v[3 + a] = Y.va[a];
+                        H->A1[a] = Y.Ai[a]; H->A1[3 + a] = Y.Aa[a];
+                    }
+                    H->tf = tf; H->h = h; H->phase = phase; H->s_old = s_old;
+                    H->t_first = t_first; H->t_last = t_last; H->slot = slot;
+                    H->n_per = n_per; H->n_coll = n_coll; H->n_tp = n_tp;
+                    H->steps_acc = steps_acc; H->steps_rej = steps_rej; H->failed = failed ? 1u : 0u;
+                    mode = MODE_IDLE;
+                }
+            }
+        }
         if (!__any_sync(IA_FULL, mode != MODE_IDLE)) {
-            if (__all_sync(IA_FULL, exhausted)) break;
+            if (wexh) break;
             continue;
         }
 
         /* ---- one DP5(4) attempt for every lane (idle lanes step a harmless dummy state) ---- */
-        bool last = false;
-        if (mode == MODE_RUN) {
-            /* clip the last step to land on t_max (R5/R8) */
-            const double rem = (P.t_max_rf - (double)n_per) * P.T_rf - tf;
-            if (h >= rem) {
-                h = rem;
-                last = true;
+        const bool run = (mode == MODE_RUN), loc = (mode == MODE_LOC);
+        /* clip the last step to land on t_max (R5/R8) */
+        const double rem = (P.t_max_rf - (double)n_per) * P.T_rf - tf;
+        const bool last = run && (h >= rem);
+        h = last ? rem : h;
+        IaVec<LPT> N;
+        IaStepOut so;
+        ia_dp5_attempt<LPT, true>(P, L, Y, tf, phase, h, N, so);
+
+        /* ---- controller, events, termination: straight-line selects; rare cases branch ---- */
+        const double hs = h; /* the step just attempted */
+        const bool accept = so.finite && (so.err.num <= P.rtol * so.err.den);
+        double xr = so.err.num * ia_rcp(so.err.den * P.rtol); /* err / rtol */
+        xr = so.finite ? xr : 1e30;
+        xr = fmax(fmin(xr, 1e30), 1e-30); /* NaN -> 1e30 (fmin returns the non-NaN operand) */
+        const double fac = 0.8 * ia_inv_fifth_root(xr); /* 0.8 (rtol/err)^(1/5) */
+        const double now = (double)n_per * P.T_rf + tf;
+        const double g = so.r2n - P.r0sq;
+        const bool g_small = fabs(g) <= P.loc_tol;
+        const bool acc = run && accept, rej = run && !accept;
+        steps_acc += acc ? 1u : 0u;
+        if (rej) ++steps_rej;
+        /* events (R6): sign changes of s = d.w at accepted-step ends */
+        const double s_prev = s_old;
+        const bool neg_old = s_prev < 0.0, neg_new = so.s_new < 0.0;
+        const bool flip = acc && (neg_old != neg_new);
+        if (flip) {
+            ++n_tp;
+            if (neg_old && so.r2n < P.rcsq) { /* a minimum of r(t) at short range: a bounce */
+                const double tc = now + (hs * s_prev) * ia_rcp(s_prev - so.s_new);
+                if (n_coll == 0u) t_first = tc;
+                t_last = tc;
+                ++n_coll;
             }
         }
-        double xn[6], vn[6], A7[6], r2n;
-        IaErr err;
-        bool finite;
-        ia_dp5_attempt(P, x, v, A1, tf, phase, h, xn, vn, A7, r2n, err, finite);
-
-        if (mode != MODE_IDLE) {
-            /* controller quantities, common to accept and reject: yq = (rtol/err)^(1/5) */
-            const bool accept = finite && (err.num <= P.rtol * err.den);
-            double xr = err.num * ia_rcp(err.den * P.rtol);
-            if (!finite) xr = 1e30;
-            xr = fmax(fmin(xr, 1e30), 1e-30); /* NaN -> 1e30 (fmin returns the non-NaN operand) */
-            const double yq = ia_inv_fifth_root(xr);
-            const double s_new = ia_sdot(xn, vn);
-            const double now = (double)n_per * P.T_rf + tf;
-            int fin = -1;          /* >= 0: terminate with this status */
-            bool fin_new = false;  /* observables from (xn, vn) instead of (x, v) */
-            double t_fin = 0.0;
-            if (mode == MODE_RUN) {
-                if (accept) {
-                    ++steps_acc;
-                    /* events (R6): sign changes of s = d.w at accepted-step ends */
-                    const bool neg_old = s_old < 0.0, neg_new = s_new < 0.0;
-                    if (neg_old != neg_new) {
-                        ++n_tp;
-                        if (neg_old && r2n < P.rcsq) {
-                            const double tc = now + h * s_old / (s_old - s_new);
-                            if (n_coll == 0) t_first = tc;
-                            t_last = tc;
-                            ++n_coll;
-                        }
-                    }
-                    if (r2n > P.r0sq && s_new > 0.0) {
-                        /* exit (R7): first upward crossing of |d| = r0; localise it by Newton on
-                         * g(hk) = |d(t_n + hk)|^2 - r0^2 over uncontrolled steps from (t_n, y_n) */
-                        const double g = r2n - P.r0sq;
-                        if (fabs(g) <= P.loc_tol) {
-                            fin = 0; fin_new = true; t_fin = now + h;
-                        } else {
-                            mode = MODE_LOC;
-                            n_loc = 0;
-                            h = h - g / (2.0 * s_new);
-                        }
-                    } else {
-                        /* commit */
-                        tf += h;
-                        if (tf >= P.T_rf) {
-                            tf -= P.T_rf;
-                            ++n_per;
-                        }
+        /* exit (R7): first upward crossing of |d| = r0, localised by Newton on
+         * g(hk) = |d(t_n + hk)|^2 - r0^2 over uncontrolled steps from (t_n, y_n) */
+        const bool exitc = acc && (so.r2n > P.r0sq) && (so.s_new > 0.0);
+        bool loc_done = false;
+        if (loc) {
+            ++n_loc;
+            loc_done = g_small || n_loc >= 8u;
+        }
+        const bool fin_exit = (exitc && g_small) || loc_done;
+        const bool newton = (exitc && !g_small) || (loc && !loc_done);
+        const bool commit = acc && !exitc;
+        const bool underflow = rej && (hs <= P.h_min);
+        /* commit the accepted step: y <- ynew, k1 <- k7 (FSAL), t <- t + h with the time kept folded (R9) */
+        {
+            const double tfn = tf + hs;
+            const bool wrap = tfn >= P.T_rf;
+            tf = commit ? (wrap ? tfn - P.T_rf : tfn) : tf;
+            n_per += (commit && wrap) ? 1u : 0u;
 #pragma unroll
-                        for (int i = 0; i < 6; ++i) {
-                            x[i] = xn[i];
-                            v[i] = vn[i];
-                            A1[i] = A7[i];
-                        }
-                        s_old = s_new;
-                        if (last) {
-                            fin = 1; t_fin = P.t_max;
-                        } else {
-                            if (!failed) h = h * fmin(5.0, 0.8 * yq);
-                            if (h > P.h_max) h = P.h_max;
-                            failed = false;
-                        }
-                    }
-                } else {
-                    ++steps_rej;
-                    if (h <= P.h_min) {
-                        fin = 2; t_fin = now;
-                    } else if (!failed) {
-                        failed = true;
-                        h = fmax(P.h_min, h * fmax(0.1, 0.8 * yq));
-                    } else {
-                        h = fmax(P.h_min, 0.5 * h);
-                    }
-                }
-                if (fin < 0 && mode == MODE_RUN &&
-                    (unsigned long long)steps_acc + (unsigned long long)steps_rej >= P.max_steps) {
-                    fin = 4;
-                    t_fin = (double)n_per * P.T_rf + tf;
-                }
-            } else { /* MODE_LOC */
-                ++n_loc;
-                const double g = r2n - P.r0sq;
-                if (fabs(g) <= P.loc_tol || n_loc >= 8) {
-                    fin = 0; fin_new = true; t_fin = now + h;
-                } else {
-                    h = h - g / (2.0 * s_new);
-                }
+            for (int a = 0; a < NA; ++a) {
+                Y.xi[a] = commit ? N.xi[a] : Y.xi[a];
+                Y.xa[a] = commit ? N.xa[a] : Y.xa[a];
+                Y.vi[a] = commit ? N.vi[a] : Y.vi[a];
+                Y.va[a] = commit ? N.va[a] : Y.va[a];
+                Y.Ai[a] = commit ? N.Ai[a] : Y.Ai[a];
+                Y.Aa[a] = commit ? N.Aa[a] : Y.Aa[a];
             }
+            if (commit) s_old = so.s_new;
+        }
+        /* step size of the next attempt (R5) */
+        {
+            const double h_acc = fmin(failed ? hs : hs * fmin(5.0, fac), P.h_max);
+            const double h_rej = fmax(P.h_min, failed ? 0.5 * hs : hs * fmax(0.1, fac));
+            h = commit ? h_acc : (rej ? h_rej : hs);
+            failed = commit ? false : (rej ? true : failed);
+        }
+        if (newton) {
+            h = hs - g * ia_rcp(2.0 * so.s_new);
+            if (exitc) n_loc = 0u;
+            mode = MODE_LOC;
+        }
+        int fin = -1; /* >= 0: terminate with this status */
+        double t_fin = now + hs;
+        if (fin_exit) {
+            fin = 0;
+        } else if (commit && last) {
+            fin = 1;
+            t_fin = P.t_max;
+        } else if (underflow) {
+            fin = 2;
+            t_fin = now;
+        } else if (run && !newton && (unsigned long long)steps_acc + (unsigned long long)steps_rej >= P.max_steps) {
+            fin = 4;
+            t_fin = (double)n_per * P.T_rf + tf;
+        }
 
+        if (__any_sync(IA_FULL, fin >= 0)) {
+            /* observables (R10) + record (a10) + ensemble reduction (a11); the velocity vectors of the
+             * terminating state are gathered by the whole warp, the group leader writes */
+            double wi[NA], wa[NA], VI[3], VA[3];
+#pragma unroll
+            for (int a = 0; a < NA; ++a) {
+                wi[a] = fin_exit ? N.vi[a] : Y.vi[a];
+                wa[a] = fin_exit ? N.va[a] : Y.va[a];
+            }
+            ia_gather3<LPT>(L, wi, VI);
+            ia_gather3<LPT>(L, wa, VA);
             if (fin >= 0) {
-                /* observables (R10) + record (a10) + ensemble reduction (a11) */
-                const double w0 = fin_new ? vn[0] : v[0], w1 = fin_new ? vn[1] : v[1], w2 = fin_new ? vn[2] : v[2];
-                const double ke = 0.5 * P.m_i * (w0 * w0 + w1 * w1 + w2 * w2);
-                if (O.records != nullptr) {
-                    ia_record r;
-                    r.ke_ion = ke;
-                    r.t_dwell = t_fin;
-                    r.t_life = (n_coll >= 2) ? (t_last - t_first) : 0.0;
-                    r.va_f[0] = fin_new ? vn[3] : v[3];
-                    r.va_f[1] = fin_new ? vn[4] : v[4];
-                    r.va_f[2] = fin_new ? vn[5] : v[5];
-                    r.n_coll = n_coll;
-                    r.n_tp = n_tp;
-                    r.steps_acc = steps_acc;
-                    r.steps_rej = (uint16_t)min(steps_rej, 65535u);
-                    r.status = (uint8_t)fin;
-                    r.n_loc = (uint8_t)n_loc;
-                    O.records[slot] = r;
-                }
-                if (O.summary != nullptr) {
-                    ia_summary *S = O.summary;
-                    atomicAdd((unsigned long long *)&S->n_done, 1ull);
-                    atomicAdd((unsigned long long *)&S->n_status[fin], 1ull);
-                    if (n_coll >= 2) atomicAdd((unsigned long long *)&S->n_complex, 1ull);
-                    atomicAdd((unsigned long long *)&S->steps_acc, (unsigned long long)steps_acc);
-                    atomicAdd((unsigned long long *)&S->steps_rej, (unsigned long long)steps_rej);
-                    atomicAdd((unsigned long long *)&S->steps_loc, (unsigned long long)n_loc);
-                    if (fin == 0) {
-                        atomicAdd(&S->sum_ke, ke);
-                        atomicAdd(&S->sum_ke2, ke * ke);
+                if (L.leader) {
+                    const double ke = (0.5 * P.m_i) * ia_dot3<true>(VI, VI);
+                    if (O.records != nullptr) {
+                        ia_record r;
+                        r.ke_ion = ke;
+                        r.t_dwell = t_fin;
+                        r.t_life = (n_coll >= 2u) ? (t_last - t_first) : 0.0;
+                        r.va_f[0] = VA[0]; r.va_f[1] = VA[1]; r.va_f[2] = VA[2];
+                        r.n_coll = n_coll;
+                        r.n_tp = n_tp;
+                        r.steps_acc = steps_acc;
+                        r.steps_rej = (uint16_t)min(steps_rej, 65535u);
+                        r.status = (uint8_t)fin;
+                        r.n_loc = (uint8_t)n_loc;
+                        O.records[slot] = r;
                     }
-                    const int bin = (n_coll == 0) ? 0 : min(32 - __clz(n_coll), IA_HIST_BINS - 1);
-                    atomicAdd((unsigned long long *)&S->hist_ncoll[bin], 1ull);
+                    if (O.summary != nullptr) {
+                        ia_summary *Sm = O.summary;
+                        atomicAdd((unsigned long long *)&Sm->n_done, 1ull);
+                        atomicAdd((unsigned long long *)&Sm->n_status[fin], 1ull);
+                        if (n_coll >= 2u) atomicAdd((unsigned long long *)&Sm->n_complex, 1ull);
+                        atomicAdd((unsigned long long *)&Sm->steps_acc, (unsigned long long)steps_acc);
+                        atomicAdd((unsigned long long *)&Sm->steps_rej, (unsigned long long)steps_rej);
+                        atomicAdd((unsigned long long *)&Sm->steps_loc, (unsigned long long)n_loc);
+                        if (S.q_in != nullptr) {
+                            atomicAdd((unsigned long long *)&Sm->n_handoff, 1ull);
+                            atomicAdd((unsigned long long *)&Sm->steps_coop,
+                                      (unsigned long long)(steps_acc + steps_rej - steps_in + n_loc));
+                        }
+                        if (fin == 0) {
+                            atomicAdd(&Sm->sum_ke, ke);
+                            atomicAdd(&Sm->sum_ke2, ke * ke);
+                        }
+                        const int bin = (n_coll == 0u) ? 0 : min(32 - __clz(n_coll), IA_HIST_BINS - 1);
+                        atomicAdd((unsigned long long *)&Sm->hist_ncoll[bin], 1ull);
+                    }
                 }
                 mode = MODE_IDLE;
             }
         }
     }
-    if (O.summary != nullptr && lane == 0) atomicMax((unsigned long long *)&O.summary->t_end_ns, ia_globaltimer());
+    if (O.summary != nullptr && lane == 0) {
+        const unsigned long long t1 = ia_globaltimer();
+        atomicMax((unsigned long long *)&O.summary->t_end_ns, t1);
+        if (S.q_in == nullptr) atomicMax((unsigned long long *)&O.summary->t_bulk_end_ns, t1);
+    }
+}
+
+/* ---- K3: verification kernels (BASELINE.json north_star: fixed-step mode, fmad off) ------------ */
+
+/* n independent uncontrolled steps: the one-step map of reading R12(i).  With LPT = 3 a warp takes ten
+ * states; every lane runs the step (shuffles) and lanes without a state of their own recompute one. */
+template <int LPT, bool FUSED>
+__global__ void ia_step_map_kernel(const __grid_constant__ IaParams P, unsigned long long n, const double *t_frac,
+                                   const double *phase, const double *y, const double *h, double *ynew,
+                                   double *err_out) {
+    constexpr int NA = 3 / LPT;
+    const unsigned lane = threadIdx.x & 31u;
+    const IaLane<LPT> L = ia_make_lane<LPT>(P, lane);
+    const unsigned long long warp = ((unsigned long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const unsigned per_warp = (LPT == 1) ? 32u : 10u;
+    unsigned long long j = warp * per_warp + (LPT == 1 ? lane : L.gbase / 3u);
+    const bool mine = L.valid && (j < n);
+    if (j >= n) j = n - 1;
+    IaVec<LPT> Y, N;
+#pragma unroll
+    for (int a = 0; a < NA; ++a) {
+        const unsigned ax = L.axis0 + a;
+        Y.xi[a] = y[j * 12 + ax];     Y.xa[a] = y[j * 12 + 3 + ax];
+        Y.vi[a] = y[j * 12 + 6 + ax]; Y.va[a] = y[j * 12 + 9 + ax];
+    }
+    const double tf = t_frac[j], ph = phase[j];
+    double D[3], r2, s;
+    ia_accel<LPT, FUSED>(P, L, Y.xi, Y.xa, ia_cos_folded(ia_fma<FUSED>(P.omega, tf, ph)), Y.Ai, Y.Aa, D, r2, s);
+    IaStepOut so;
+    ia_dp5_attempt<LPT, FUSED>(P, L, Y, tf, ph, h[j], N, so);
+    if (!mine) return;
+#pragma unroll
+    for (int a = 0; a < NA; ++a) {
+        const unsigned ax = L.axis0 + a;
+        ynew[j * 12 + ax] = N.xi[a];     ynew[j * 12 + 3 + ax] = N.xa[a];
+        ynew[j * 12 + 6 + ax] = N.vi[a]; ynew[j * 12 + 9 + ax] = N.va[a];
+    }
+    if (err_out != nullptr && L.leader)
+        err_out[j] = so.finite ? so.err.num / so.err.den : __longlong_as_double(0x7ff8000000000000ll);
+}
+
+/* nsteps uncontrolled steps of one trajectory, every state written out (reading R12(ii)); one warp,
+ * every group integrates the same trajectory and group 0 writes */
+template <int LPT, bool FUSED>
+__global__ void ia_trace_kernel(const __grid_constant__ IaParams P, IaY12 y0, double phase, double h,
+                                unsigned nsteps, double *states) {
+    constexpr int NA = 3 / LPT;
+    const unsigned lane = threadIdx.x & 31u;
+    const IaLane<LPT> L = ia_make_lane<LPT>(P, lane);
+    const bool writer = (lane < (unsigned)LPT);
+    IaVec<LPT> Y, N;
+#pragma unroll
+    for (int a = 0; a < NA; ++a) {
+        const unsigned ax = L.axis0 + a;
+        Y.xi[a] = ia_sel3(y0.y[0], y0.y[1], y0.y[2], ax);  Y.xa[a] = ia_sel3(y0.y[3], y0.y[4], y0.y[5], ax);
+        Y.vi[a] = ia_sel3(y0.y[6], y0.y[7], y0.y[8], ax);  Y.va[a] = ia_sel3(y0.y[9], y0.y[10], y0.y[11], ax);
+    }
+    double tf = 0.0;
+    unsigned n_per = 0;
+    auto store = [&](unsigned row, double t) {
+        if (!writer) return;
+        double *o = states + (unsigned long long)row * 13;
+        if (L.leader) o[0] = t;
+#pragma unroll
+        for (int a = 0; a < NA; ++a) {
+            const unsigned ax = L.axis0 + a;
+            o[1 + ax] = Y.xi[a]; o[4 + ax] = Y.xa[a]; o[7 + ax] = Y.vi[a]; o[10 + ax] = Y.va[a];
+        }
+    };
+    store(0, 0.0);
+    double D[3], r2, s;
+    ia_accel<LPT, FUSED>(P, L, Y.xi, Y.xa, ia_cos_folded(phase), Y.Ai, Y.Aa, D, r2, s);
+    for (unsigned n = 0; n < nsteps; ++n) {
+        IaStepOut so;
+        ia_dp5_attempt<LPT, FUSED>(P, L, Y, tf, phase, h, N, so);
+        tf += h;
+        if (tf >= P.T_rf) {
+            tf -= P.T_rf;
+            ++n_per;
+        }
+        Y = N;
+        store(n + 1, (double)n_per * P.T_rf + tf);
+    }
 }
 
 /* ---- host launchers ------------------------------------------------------------------------ */
 
-cudaError_t ia_launch_persistent(const IaParams &P, const IaGen &G, const IaOut &O, unsigned long long *counter,
-                                 unsigned long long warn, int grid_blocks, cudaStream_t st) {
-    ia_persistent_kernel<<<grid_blocks, IA_THREADS, 0, st>>>(P, G, O, counter, warn);
+cudaError_t ia_launch_persistent(int lanes_per_traj, const IaParams &P, const IaGen &G, const IaOut &O,
+                                 const IaSched &S, int grid_blocks, cudaStream_t st) {
+    if (lanes_per_traj == 1)
+        ia_persistent_kernel<1><<<grid_blocks, IA_THREADS, 0, st>>>(P, G, O, S);
+    else
+        ia_persistent_kernel<3><<<grid_blocks, IA_THREADS, 0, st>>>(P, G, O, S);
     return cudaGetLastError();
 }
 
-cudaError_t ia_persistent_info(int device, int *blocks_per_sm, int *threads_per_block, int *regs, int *local_bytes) {
-    (void)device;
+cudaError_t ia_persistent_info(int lanes_per_traj, int *blocks_per_sm, int *threads_per_block, int *regs,
+                               int *local_bytes) {
+    const void *fn = lanes_per_traj == 1 ? (const void *)ia_persistent_kernel<1> : (const void *)ia_persistent_kernel<3>;
     cudaFuncAttributes fa;
-    cudaError_t e = cudaFuncGetAttributes(&fa, ia_persistent_kernel);
+    cudaError_t e = cudaFuncGetAttributes(&fa, fn);
     if (e != cudaSuccess) return e;
     int nb = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, ia_persistent_kernel, IA_THREADS, 0);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, fn, IA_THREADS, 0);
     if (e != cudaSuccess) return e;
     *blocks_per_sm = nb;
     *threads_per_block = IA_THREADS;
@@ -394,5 +590,29 @@ cudaError_t ia_launch_generate(const IaParams &P, const IaGen &G, double *ic_dum
     return cudaGetLastError();
 }
 
-#define IA_VARIANT fma
-#include "ia_verify.cuh"
+cudaError_t ia_launch_step_map(int variant, const IaParams &P, unsigned long long n, const double *t_frac,
+                               const double *phase, const double *y, const double *h, double *ynew, double *err,
+                               cudaStream_t st) {
+    if (n == 0) return cudaSuccess;
+    const unsigned threads = 64;
+    const unsigned long long per_block = (variant == IA_ARITH_FMA_COOP) ? 20ull : 64ull;
+    const unsigned blocks = (unsigned)((n + per_block - 1) / per_block);
+    if (variant == IA_ARITH_NOFMA)
+        ia_step_map_kernel<1, false><<<blocks, threads, 0, st>>>(P, n, t_frac, phase, y, h, ynew, err);
+    else if (variant == IA_ARITH_FMA)
+        ia_step_map_kernel<1, true><<<blocks, threads, 0, st>>>(P, n, t_frac, phase, y, h, ynew, err);
+    else
+        ia_step_map_kernel<3, true><<<blocks, threads, 0, st>>>(P, n, t_frac, phase, y, h, ynew, err);
+    return cudaGetLastError();
+}
+
+cudaError_t ia_launch_trace(int variant, const IaParams &P, IaY12 y0, double phase, double h, unsigned nsteps,
+                            double *states, cudaStream_t st) {
+    if (variant == IA_ARITH_NOFMA)
+        ia_trace_kernel<1, false><<<1, 32, 0, st>>>(P, y0, phase, h, nsteps, states);
+    else if (variant == IA_ARITH_FMA)
+        ia_trace_kernel<1, true><<<1, 32, 0, st>>>(P, y0, phase, h, nsteps, states);
+    else
+        ia_trace_kernel<3, true><<<1, 32, 0, st>>>(P, y0, phase, h, nsteps, states);
+    return cudaGetLastError();
+}

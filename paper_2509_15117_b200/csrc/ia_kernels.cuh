@@ -27,25 +27,43 @@ struct IaOut {
     double *ic_dump;
 };
 
-/* persistent propagation kernel: returns cudaError of the launch */
-cudaError_t ia_launch_persistent(const IaParams &P, const IaGen &G, const IaOut &O, unsigned long long *counter,
-                                 unsigned long long warn, int grid_blocks, cudaStream_t st);
-cudaError_t ia_persistent_info(int device, int *blocks_per_sm, int *threads_per_block, int *regs, int *local_bytes);
+/* A trajectory in flight, as the bulk kernel hands it to the straggler kernel (256 bytes). */
+struct IaHand {
+    double x[6], v[6], A1[6]; /* r_i, r_a | v_i, v_a | FSAL accelerations */
+    double tf, h, phase, s_old, t_first, t_last;
+    unsigned long long slot;
+    unsigned n_per, n_coll, n_tp, steps_acc, steps_rej, failed;
+    unsigned long long pad[4];
+};
+static_assert(sizeof(IaHand) == 256, "IaHand is 256 bytes");
+
+/* where a persistent kernel takes its work from and where unfinished work goes */
+struct IaSched {
+    unsigned long long *counter;     /* work counter of this launch (zeroed by the host)                 */
+    const IaHand *q_in;              /* non-NULL: resume trajectories from this queue instead of generating */
+    const unsigned long long *n_in;  /* ... their number (device memory, written by the producing kernel) */
+    IaHand *q_out;                   /* non-NULL: hand unfinished trajectories over to this queue ...     */
+    unsigned long long *n_out;       /* ... counting them here                                           */
+    int handoff_lanes;               /* ... once the counter is empty and <= this many lanes of a warp run */
+    unsigned long long warn;
+};
+
+/* persistent propagation kernels: lanes_per_traj = 1 (bulk) or 3 (straggler / cooperative layout) */
+cudaError_t ia_launch_persistent(int lanes_per_traj, const IaParams &P, const IaGen &G, const IaOut &O,
+                                 const IaSched &S, int grid_blocks, cudaStream_t st);
+cudaError_t ia_persistent_info(int lanes_per_traj, int *blocks_per_sm, int *threads_per_block, int *regs,
+                               int *local_bytes);
 cudaError_t ia_launch_generate(const IaParams &P, const IaGen &G, double *ic_dump, cudaStream_t st);
 
-/* verification kernels, two arithmetic variants */
-cudaError_t ia_launch_step_map_fma(const IaParams &P, unsigned long long n, const double *t_frac, const double *phase,
-                                   const double *y, const double *h, double *ynew, double *err, cudaStream_t st);
-cudaError_t ia_launch_step_map_nofma(const IaParams &P, unsigned long long n, const double *t_frac,
-                                     const double *phase, const double *y, const double *h, double *ynew,
-                                     double *err, cudaStream_t st);
+/* verification kernels; variant = ia_arith (include/ia.h) */
+cudaError_t ia_launch_step_map(int variant, const IaParams &P, unsigned long long n, const double *t_frac,
+                               const double *phase, const double *y, const double *h, double *ynew, double *err,
+                               cudaStream_t st);
 struct IaY12 {
     double y[12];
 };
-cudaError_t ia_launch_trace_fma(const IaParams &P, IaY12 y0, double phase, double h, unsigned nsteps, double *states,
-                                cudaStream_t st);
-cudaError_t ia_launch_trace_nofma(const IaParams &P, IaY12 y0, double phase, double h, unsigned nsteps,
-                                  double *states, cudaStream_t st);
+cudaError_t ia_launch_trace(int variant, const IaParams &P, IaY12 y0, double phase, double h, unsigned nsteps,
+                            double *states, cudaStream_t st);
 
 /* DFMA peak microbenchmark */
 cudaError_t ia_run_fp64_peak(int device, double target_ms, double *tflops, double *elapsed_ms);

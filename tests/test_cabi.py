@@ -49,7 +49,9 @@ def test_strerror_and_null_arguments():
     assert L.ia_trace(None, None, 0.0, 1.0, 1, None, 0, None) == P.IA_EINVAL
     assert L.ia_destroy(None) == P.IA_EINVAL
     assert L.ia_get_derived(None, None) == P.IA_EINVAL
-    assert L.ia_get_kernel_info(None, None, None, None, None) == P.IA_EINVAL
+    assert L.ia_get_kernel_info(None, 0, None, None, None, None) == P.IA_EINVAL
+    assert L.ia_set_handoff(None, 8) == P.IA_EINVAL
+    assert L.ia_get_last_timing(None, None, None) == P.IA_EINVAL
     assert L.ia_fp64_peak(0, 10.0, None, None) == P.IA_EINVAL
     assert P.ia_last_error(None) == ""
 

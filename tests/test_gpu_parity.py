@@ -95,9 +95,9 @@ def _sampled_states(cell, n_traj=6, seed=3):
     return tf, ph, y, h
 
 
-@pytest.mark.parametrize("use_fma", [False, True])
+@pytest.mark.parametrize("variant", [0, 1, 2])   # ia_arith: fmad off / production one-lane / production three-lane
 @pytest.mark.parametrize("which", ["config0", "config1"])
-def test_one_step_map_1e12(P, which, use_fma):
+def test_one_step_map_1e12(P, which, variant):
     cell = I.config0() if which == "config0" else I.config1(64)
     tf, ph, y, h = _sampled_states(cell)
     assert len(y) > 300 and np.linalg.norm(y[:, 3:6] - y[:, 0:3], axis=1).min() < 80.0  # reaches the well
@@ -107,9 +107,9 @@ def test_one_step_map_1e12(P, which, use_fma):
         ref[k] = yn
         eref[k] = O.err_norm(cell.params, y[k], yn, e)
     with P.Context(cell.params) as ctx:
-        got, err = ctx.step_map(tf, ph, y, h, use_fma=use_fma)
+        got, err = ctx.step_map(tf, ph, y, h, variant=variant)
     rel = block_rel(got, ref, 1e-3 * np.linalg.norm(y[:, 9:12], axis=1).max())
-    print(f"\none-step map {which} fma={use_fma}: n={len(y)} max block rel diff {rel.max(axis=0)}")
+    print(f"\none-step map {which} variant={variant}: n={len(y)} max block rel diff {rel.max(axis=0)}")
     assert rel.max() <= 1e-12
     # the error norm is a sum with cancelling weights (sum E_l = 0): agreement to ~1e-6 of itself
     assert np.max(np.abs(err - eref) / eref) < 1e-5
@@ -127,9 +127,13 @@ def test_mixed_random_states_one_step(P):
     h = 1e-3 * T * np.clip(r / 1000.0, 1e-3, 1.0)
     ref = np.stack([O.step(cell.params, tf[k], ph[k], y[k], h[k])[0] for k in range(n)])
     with P.Context(cell.params) as ctx:
-        for fma in (False, True):
-            got, _ = ctx.step_map(tf, ph, y, h, use_fma=fma)
+        out = {}
+        for variant in (0, 1, 2):
+            got, err = ctx.step_map(tf, ph, y, h, variant=variant)
             assert block_rel(got, ref, 1e-9).max() <= 1e-12
+            out[variant] = (got, err)
+    # the one-lane and the three-lane layout run the same IEEE operations per component: bit-identical
+    assert np.array_equal(out[1][0], out[2][0]) and np.array_equal(out[1][1], out[2][1])
 
 
 def test_cumulative_trace(P):
@@ -144,8 +148,10 @@ def test_cumulative_trace(P):
     rmin_at = np.argmin(np.linalg.norm(ref[:, 4:7] - ref[:, 1:4], axis=1))
     assert 0 < rmin_at < nsteps - 50
     with P.Context(cell.params) as ctx:
-        for fma in (False, True):
-            got = ctx.trace(y0[0], ph[0], h, nsteps, use_fma=fma)
+        traces = {}
+        for fma in (0, 1, 2):
+            got = ctx.trace(y0[0], ph[0], h, nsteps, variant=fma)
+            traces[fma] = got
             assert np.max(np.abs(got[:, 0] - ref[:, 0]) / np.maximum(ref[:, 0], h)) < 1e-14
             rel = block_rel(got[:, 1:], ref[:, 1:], 1e-3 * np.linalg.norm(ref[:, 10:13], axis=1).max()).max(axis=1)
             over = np.nonzero(rel > 1e-12)[0]
@@ -154,6 +160,7 @@ def test_cumulative_trace(P):
                   f"{rel[:rmin_at - 20].max():.2e}, overall {rel.max():.2e}; 1e-12 first exceeded at step {first}")
             assert rel[:rmin_at - 20].max() <= 1e-12
             assert rel.max() <= 1e-7   # after the bounce: amplified energy round-off, (D_e/E) eps sqrt(N) (R12(ii))
+    assert np.array_equal(traces[1], traces[2])   # both layouts, 1800 steps: bit-identical
 
 
 @pytest.mark.parametrize("axis", [0, 1, 2])
@@ -172,6 +179,55 @@ def test_mirror_symmetry_is_bitwise_on_the_gpu(P, axis):
     assert np.array_equal(a["va_f"] * flip, b["va_f"])
     for f in ("ke_ion", "t_dwell", "n_coll", "n_tp", "steps_acc", "steps_rej", "status"):
         assert np.array_equal(a[f], b[f])
+
+
+# ---------------------------------------------------------------------------------------------
+# the two persistent kernels give the same records bit for bit, wherever a trajectory is handed over
+# ---------------------------------------------------------------------------------------------
+_REC_FIELDS = ("ke_ion", "t_dwell", "t_life", "va_f", "n_coll", "n_tp", "steps_acc", "steps_rej", "status", "n_loc")
+
+
+def _assert_records_identical(a, b):
+    for f in _REC_FIELDS:
+        assert np.array_equal(a[f], b[f]), f
+
+
+@pytest.mark.parametrize("which", ["config0", "config1", "config4"])
+def test_bulk_coop_and_handoff_paths_are_bit_identical(P, which):
+    """IA_PATH_BULK_ONLY (one lane per trajectory to the end), IA_PATH_COOP_ONLY (three lanes per trajectory
+    from the first step) and IA_PATH_AUTO with hand-over thresholds 4, 16 and 32 lanes: identical records,
+    chaotic trajectories included (config 1 at 48x48 = 2,304 trajectories, a ragged 72 warps; config 4's
+    Philox stream)."""
+    if which == "config0":
+        cell = I.config0()
+    elif which == "config1":
+        cell = I.config1(48)
+        cell = replace(cell, params=replace(cell.params, t_max_rf=300.0))
+    else:
+        cell = I.config4(n_total=1500, batch=1500)[0]
+        cell = replace(cell, params=replace(cell.params, t_max_rf=300.0))
+    runs = {}
+    with P.Context(cell.params) as ctx:
+        runs["bulk"], s_bulk, _ = ctx.run_sync(replace(cell.launch, path=1))
+        runs["coop"], s_coop, _ = ctx.run_sync(replace(cell.launch, path=2))
+        for lanes in (4, 16, 32):
+            ctx.set_handoff(lanes)
+            runs[f"auto{lanes}"], s_auto, _ = ctx.run_sync(replace(cell.launch, path=0))
+            assert int(s_auto["n_done"]) == cell.launch.n
+            if lanes == 32:
+                assert int(s_auto["n_handoff"]) > 0 and int(s_auto["steps_coop"]) > 0   # the hand-over did happen
+        ctx.set_handoff(0)
+        runs["auto0"], s0, _ = ctx.run_sync(replace(cell.launch, path=0))
+        assert int(s0["n_handoff"]) == 0
+    assert int(s_bulk["n_done"]) == cell.launch.n == int(s_coop["n_done"])
+    assert int(s_bulk["n_handoff"]) == 0 and int(s_coop["n_handoff"]) == 0
+    if which != "config0":
+        assert (runs["bulk"]["n_coll"] >= 2).sum() > 100      # chaotic trajectories are in the sample
+    for k, r in runs.items():
+        _assert_records_identical(runs["bulk"], r)
+    for f in ("n_done", "n_complex", "steps_acc", "steps_rej", "steps_loc"):
+        assert int(s_bulk[f]) == int(s_coop[f]) == int(s_auto[f])
+    assert np.array_equal(s_bulk["hist_ncoll"], s_coop["hist_ncoll"])
 
 
 # ---------------------------------------------------------------------------------------------
