@@ -22,6 +22,10 @@ import sys
 import tempfile
 import time
 
+# One hardware work queue per stream: with the default of 8, the straggler streams of a deep pipeline would share
+# queues and their kernels would serialise behind one another (must be set before CUDA is initialised).
+os.environ.setdefault("CUDA_DEVICE_MAX_CONNECTIONS", "32")
+
 ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
@@ -32,17 +36,17 @@ import ia_inputs as I  # noqa: E402
 
 METRIC = "trajectories/s"
 # Algorithmic FP64 flops per ATTEMPTED RK step (FMA = 2), counted from the formulas of the
-# Nystrom-collapsed DP5(4) step in DESIGN.md section "Roofline": coefficient products 35, cosines 165,
+# Nystrom-collapsed DP5(4) step in DESIGN.md section "Roofline": coefficient products 35, five cosines 135,
 # stage sums 300, six accelerations 234, d.w 8, error sums 120, norm cross-products 22,
-# controller / time keeping 37.
-FLOP_PER_STEP = 921.0
+# controller / time keeping 32.
+FLOP_PER_STEP = 886.0
 ORACLE_SAMPLE_EVERY = 8   # cpu_baseline: every 8th grid point in theta and phi (64x64 = 4,096 trajectories)
 
 
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=2)
+    ap.add_argument("--steps", type=int, default=8)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--n-side", type=int, default=512)
@@ -56,6 +60,9 @@ def parse():
     ap.add_argument("--handoff", type=int, default=-1,
                     help="hand-over threshold of the bulk kernel in lanes (0 = bulk kernel only; default: the library's)")
     ap.add_argument("--path", type=int, default=0, help="ia_path: 0 production kernel pair, 1 bulk only, 2 cooperative only")
+    ap.add_argument("--pipeline", type=int, default=16,
+                    help="ia_set_pipeline depth: how many passes may still be finishing their longest trajectories on "
+                         "the library's straggler streams while later passes start (0 = strictly one pass after another)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -229,64 +236,70 @@ def run_ours(args):
     ctx = P.Context(cell.params, device=local)
     if args.handoff >= 0:
         ctx.set_handoff(args.handoff)
+    depth = max(0, min(args.pipeline, 16))
+    ctx.set_pipeline(depth)
     launch = dataclasses.replace(launch, path=args.path)
     info = ctx.kernel_info
-    rec = torch.empty(n * P.RECORD_BYTES, dtype=torch.uint8, device=dev)
+    nbuf = min(K, max(depth, 1))                 # passes in flight never share an output buffer
+    recs_d = [torch.empty(n * P.RECORD_BYTES, dtype=torch.uint8, device=dev) for _ in range(nbuf)]
     summaries = torch.zeros((W + K, P.SUMMARY_BYTES), dtype=torch.uint8, device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
 
     for w in range(W):
-        ctx.run(launch, records=rec, summary=summaries[w])
+        ctx.run(launch, records=recs_d[w % nbuf], summary=summaries[w])
         flush.fill_(w)
+    ctx.join()
     barrier()
     clocks = ClockSampler(local)
     clocks.start()
-    kernel_times = []
+    ev0.record()
     for k in range(K):
-        ev[k][0].record()
-        ctx.run(launch, records=rec, summary=summaries[W + k])     # one step = bulk kernel + straggler kernel
-        ev[k][1].record()
-        kernel_times.append(ctx.last_timing)                       # the library's own events around each kernel
+        # one step = one pass over the grid = bulk kernel + straggler kernel (the latter on the library's
+        # own stream when depth > 0, so that pass k+1 starts while pass k's longest trajectories finish)
+        ctx.run(launch, records=recs_d[k % nbuf], summary=summaries[W + k])
         flush.fill_(k)                                             # L2 flush between timed iterations
+    ctx.join()                                                     # the stream waits for every straggler kernel
+    ev1.record()
     barrier()
     clk = clocks.stop()
-    step_ms = [a.elapsed_time(b) for a, b in ev]
-    total_s = D.all_reduce_max(sum(step_ms) * 1e-3, dev)
+    total_s = D.all_reduce_max(ev0.elapsed_time(ev1) * 1e-3, dev)
+    kernel_times = [ctx.timing(back) for back in range(min(K, max(depth, 1)))]   # the library's own CUDA events
     summ = P.view_summary(summaries[W + K - 1])
     bulk_ms = float(np.mean([t["bulk_ms"] for t in kernel_times]))
     coop_ms = float(np.mean([t["coop_ms"] for t in kernel_times]))
     attempted = int(summ["steps_acc"]) + int(summ["steps_rej"]) + int(summ["steps_loc"])
     steps_coop = int(summ["steps_coop"])
-    recs = P.view_records(rec, n)
+    recs = P.view_records(recs_d[(K - 1) % nbuf], n)
     longest = int((recs["steps_acc"].astype(np.int64) + recs["steps_rej"]).max())
     tot = D.all_reduce_summary(summ, dev)
     attempted_all = tot["steps_acc"] + tot["steps_rej"] + tot["steps_loc"]
     value = world * n * K / total_s
+    step_avg_ms = 1e3 * total_s / K
 
-    # end to end through ia_run_host: explicit initial conditions in pinned host memory -> device,
-    # records + summary -> pinned host memory, all inside the timed region
+    # end to end through the host entry points: explicit initial conditions in pinned host memory -> device,
+    # records + summary -> pinned host memory, all inside the timed region (ia_submit_host x K, ia_wait)
     e2e = None
     if not args.no_e2e:
         ic = ctx.generate(launch)                                   # untimed: the inputs of the e2e leg
         y0 = torch.from_numpy(np.ascontiguousarray(ic[:, :12])).pin_memory()
         ph = torch.from_numpy(np.ascontiguousarray(ic[:, 12])).pin_memory()
-        rec_h = torch.empty(n * P.RECORD_BYTES, dtype=torch.uint8).pin_memory()
-        sum_h = torch.zeros(P.SUMMARY_BYTES, dtype=torch.uint8).pin_memory()
+        rec_h = [torch.empty(n * P.RECORD_BYTES, dtype=torch.uint8).pin_memory() for _ in range(nbuf)]
+        sum_h = [torch.zeros(P.SUMMARY_BYTES, dtype=torch.uint8).pin_memory() for _ in range(nbuf)]
         lx = I.Launch(mode=I.MODE_EXPLICIT, n=n)
         cl = P.make_launch(lx, y0, ph)
-        P.ia_run_host(ctx.handle, cl, rec_h, sum_h)                 # warm-up (staging allocation)
+        P.ia_run_host(ctx.handle, cl, rec_h[0], sum_h[0])           # warm-up (staging allocation)
         barrier()
         t0 = time.perf_counter()
         for k in range(K):
-            P.ia_run_host(ctx.handle, cl, rec_h, sum_h)             # synchronous
-        torch.cuda.synchronize(dev)
+            P.ia_submit_host(ctx.handle, cl, rec_h[k % nbuf], sum_h[k % nbuf])
+        ctx.wait()                                                  # blocks until every copy back has landed
         e2e_s = D.all_reduce_max(time.perf_counter() - t0, dev)
-        done = int(sum_h.numpy().view(P.SUMMARY_DTYPE)[0]["n_done"])
+        done = int(sum_h[(K - 1) % nbuf].numpy().view(P.SUMMARY_DTYPE)[0]["n_done"])
         assert done == n, (done, n)
         e2e = {"value": world * n * K / e2e_s, "unit": "trajectories/s",
                "h2d_bytes_per_step": int(y0.numel() * 8 + ph.numel() * 8),
-               "d2h_bytes_per_step": int(rec_h.numel() + sum_h.numel()), "ms_per_step": 1e3 * e2e_s / K}
+               "d2h_bytes_per_step": int(rec_h[0].numel() + sum_h[0].numel()), "ms_per_step": 1e3 * e2e_s / K}
     ctx.close()
     if world > 1:
         dist.barrier(device_ids=[local])
@@ -298,13 +311,13 @@ def run_ours(args):
     # roofline of the kernel that does the arithmetic: the bulk kernel (one lane per trajectory) over its own
     # launch duration; the steps the straggler kernel took are not counted for it
     achieved_tflops = FLOP_PER_STEP * (attempted - steps_coop) / (bulk_ms * 1e-3) / 1e12
-    step_avg_ms = float(np.mean(step_ms))
     line = {
         "metric": METRIC, "value": value, "unit": "trajectories/s", "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": 1e3 * total_s / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": cell.name, "trajectories_per_step_per_gpu": n, "parallelism": f"dp{world}",
                    "l2": "flushed between timed iterations (256 MiB write); the kernel reads no input arrays",
+                   "pipeline_depth": depth,
                    "rtol": cell.params.rtol, "atol": cell.params.atol, "t_max_rf": cell.params.t_max_rf},
         "rk_steps_per_s": attempted_all * K / total_s,
         "rk_steps_per_pass": attempted_all,

@@ -25,6 +25,7 @@
  *   - Every function returns IA_OK (0) or a negative ia_status; on failure nothing was launched.
  *     A failed *trajectory* is not a call error: see ia_record.status.
  *   - A ctx is not thread-safe.  Two ctxs may run concurrently on different streams.
+ *   - ia_destroy waits for the runs still in flight on the ctx.
  */
 #ifndef IA_H
 #define IA_H
@@ -163,6 +164,27 @@ int ia_run(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *outputs, void
  * overwritten (not accumulated).  This is the end-to-end entry bench.py times. */
 int ia_run_host(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *host_outputs);
 
+/* Pipelining of successive runs.  Trajectory lengths are power-law distributed
+ * (PAPER.md:40): the last few trajectories of a launch take 10^3 times longer than the median, and a
+ * trajectory is a serial chain.  With depth d > 0 (at most 16) the straggler kernel of a run goes to a
+ * ctx-owned stream, so the caller's stream is free for the bulk kernel of the next run
+ * while up to d earlier runs finish their longest trajectories; run number d+1 waits (on the device)
+ * for the oldest one.  depth 0 (the default) keeps both kernels on the caller's stream.
+ * With depth > 0 the outputs of ia_run are valid only after ia_join: it makes `cuda_stream` wait, on
+ * the device, for every straggler kernel enqueued so far (the host does not block).
+ * ia_set_pipeline synchronises with the runs in flight; it allocates d hand-over queues (IA_ENOMEM).
+ * Streams sharing a hardware work queue serialise: for d > 6 start the process with
+ * CUDA_DEVICE_MAX_CONNECTIONS >= d + 2 in its environment (the CUDA default is 8). */
+int ia_set_pipeline(ia_ctx *ctx, int depth);
+int ia_join(ia_ctx *ctx, void *cuda_stream);
+
+/* Asynchronous form of ia_run_host: enqueues the copies in, the kernels and the copies back on
+ * ctx-owned streams and returns; host buffers must be page-locked for the copies to overlap and stay
+ * untouched until ia_wait, which blocks the host until every run submitted on this ctx (either way)
+ * has finished.  With ia_set_pipeline(d) up to d submitted runs overlap. */
+int ia_submit_host(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *host_outputs);
+int ia_wait(ia_ctx *ctx);
+
 /* Generator only (R1-R3): ic_dump is a DEVICE buffer [n][14]. */
 int ia_generate(ia_ctx *ctx, const ia_launch *launch, double *ic_dump, void *cuda_stream);
 
@@ -201,9 +223,13 @@ int ia_get_kernel_info(const ia_ctx *ctx, int kernel, int *warps_per_sm, int *n_
  * is 16: the cooperative kernel with ten trajectories per warp does the work of ~18 bulk lanes). */
 int ia_set_handoff(ia_ctx *ctx, int lanes);
 
-/* Device times of the most recent ia_run / ia_run_host of this ctx, from CUDA events the library
- * records on the launch stream around its kernels: bulk kernel and cooperative kernel, in ms.
- * Synchronises with the end of that run.  Host pointers. */
+/* Device times of a run of this ctx, from CUDA events the library records on the launch streams
+ * around its kernels: bulk kernel (start -> its end) and cooperative kernel (end of the bulk kernel ->
+ * its end, which with a pipeline includes any wait for free SMs), in ms.  runs_back = 0 is the most
+ * recent run, 1 the one before ...; only the last max(depth, 1) runs are on record (IA_EINVAL
+ * otherwise).  Synchronises with the end of that run.  Host pointers.
+ * ia_get_last_timing(ctx, ...) = ia_get_timing(ctx, 0, ...). */
+int ia_get_timing(ia_ctx *ctx, int runs_back, double *bulk_ms, double *coop_ms);
 int ia_get_last_timing(ia_ctx *ctx, double *bulk_ms, double *coop_ms);
 
 /* FP64 FMA peak microbenchmark (the roofline denominator): runs independent DFMA chains on every SM

@@ -13,10 +13,16 @@ is a small convenience wrapper that owns one ``ia_ctx`` handle.
 from __future__ import annotations
 
 import ctypes as C
+import os
 from pathlib import Path
 from typing import Optional
 
 import numpy as np
+
+# ia_set_pipeline(d) runs up to d straggler kernels on streams of their own; CUDA maps streams onto
+# CUDA_DEVICE_MAX_CONNECTIONS hardware queues (default 8) and streams sharing a queue serialise.  Only
+# effective when set before the process initialises CUDA, hence here at import.
+os.environ.setdefault("CUDA_DEVICE_MAX_CONNECTIONS", "32")
 
 _HERE = Path(__file__).resolve().parent
 LIB_PATH = _HERE / "libia_b200.so"
@@ -29,8 +35,8 @@ IA_HIST_BINS = 32
 
 # every symbol include/ia.h declares (tests/test_cabi.py checks the library exports each of them)
 EXPORTS = ("ia_create", "ia_run", "ia_run_host", "ia_generate", "ia_step_map", "ia_trace", "ia_get_derived",
-           "ia_get_kernel_info", "ia_set_handoff", "ia_get_last_timing", "ia_fp64_peak", "ia_destroy", "ia_strerror",
-           "ia_last_error")
+           "ia_get_kernel_info", "ia_set_handoff", "ia_get_last_timing", "ia_get_timing", "ia_set_pipeline", "ia_join",
+           "ia_submit_host", "ia_wait", "ia_fp64_peak", "ia_destroy", "ia_strerror", "ia_last_error")
 
 
 class IaError(RuntimeError):
@@ -107,6 +113,11 @@ def load() -> C.CDLL:
     L.ia_get_kernel_info.argtypes = [vp, C.c_int, ip, ip, ip, ip]
     L.ia_set_handoff.argtypes = [vp, C.c_int]
     L.ia_get_last_timing.argtypes = [vp, dp, dp]
+    L.ia_get_timing.argtypes = [vp, C.c_int, dp, dp]
+    L.ia_set_pipeline.argtypes = [vp, C.c_int]
+    L.ia_join.argtypes = [vp, vp]
+    L.ia_submit_host.argtypes = [vp, C.POINTER(ia_launch), C.POINTER(ia_outputs)]
+    L.ia_wait.argtypes = [vp]
     L.ia_fp64_peak.argtypes = [C.c_int, C.c_double, dp, dp]
     L.ia_destroy.argtypes = [vp]
     L.ia_strerror.argtypes = [C.c_int]
@@ -239,11 +250,37 @@ def ia_set_handoff(handle, lanes: int) -> None:
     _check(load().ia_set_handoff(handle, int(lanes)), handle)
 
 
+def ia_get_timing(handle, runs_back: int = 0) -> dict:
+    """Device times (ms) of the two kernels of a recent run on this ctx (0 = the last); synchronises with it."""
+    a, b = C.c_double(), C.c_double()
+    _check(load().ia_get_timing(handle, int(runs_back), C.byref(a), C.byref(b)), handle)
+    return {"bulk_ms": a.value, "coop_ms": b.value}
+
+
 def ia_get_last_timing(handle) -> dict:
-    """Device times (ms) of the two kernels of the most recent run on this ctx; synchronises with it."""
     a, b = C.c_double(), C.c_double()
     _check(load().ia_get_last_timing(handle, C.byref(a), C.byref(b)), handle)
     return {"bulk_ms": a.value, "coop_ms": b.value}
+
+
+def ia_set_pipeline(handle, depth: int) -> None:
+    """Up to `depth` runs finish their longest trajectories on ctx-owned streams while later runs start."""
+    _check(load().ia_set_pipeline(handle, int(depth)), handle)
+
+
+def ia_join(handle, stream=None) -> None:
+    """Makes `stream` (default: torch's current stream) wait on the device for every straggler kernel enqueued."""
+    _check(load().ia_join(handle, _stream_handle(stream)), handle)
+
+
+def ia_submit_host(handle, launch: ia_launch, records=None, summary=None, ic_dump=None) -> None:
+    """Asynchronous ia_run_host: pinned host buffers, valid after ia_wait."""
+    out = ia_outputs(_ptr(records), _ptr(summary), _ptr(ic_dump))
+    _check(load().ia_submit_host(handle, C.byref(launch), C.byref(out)), handle)
+
+
+def ia_wait(handle) -> None:
+    _check(load().ia_wait(handle), handle)
 
 
 def ia_fp64_peak(device: int = 0, target_ms: float = 200.0) -> dict:
@@ -298,6 +335,18 @@ class Context:
     @property
     def last_timing(self) -> dict:
         return ia_get_last_timing(self.handle)
+
+    def timing(self, runs_back: int = 0) -> dict:
+        return ia_get_timing(self.handle, runs_back)
+
+    def set_pipeline(self, depth: int) -> None:
+        ia_set_pipeline(self.handle, depth)
+
+    def join(self, stream=None) -> None:
+        ia_join(self.handle, stream)
+
+    def wait(self) -> None:
+        ia_wait(self.handle)
 
     def alloc(self, n: int, ic_dump: bool = False):
         """(records uint8[n*64], summary uint8[512] zeroed, ic_dump float64[n,14] or None) on the device."""

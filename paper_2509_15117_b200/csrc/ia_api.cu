@@ -23,6 +23,18 @@ struct IaKernelInfo {
     int blocks_per_sm = 0, threads_per_block = 0, regs = 0, local_bytes = 0;
 };
 
+#define IA_PIPE_MAX 16
+
+struct IaSlot {
+    IaHand *queue = nullptr;
+    cudaStream_t tail = nullptr;             /* non-blocking stream of the straggler kernel               */
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr}; /* start, bulk end, run end, host copies done */
+    bool used = false;                       /* ev[2] has been recorded                                    */
+    bool host_used = false;                  /* ev[3] has been recorded                                    */
+    void *stage = nullptr;                   /* device staging of the host entry points                    */
+    size_t stage_bytes = 0;
+};
+
 struct ia_ctx {
     int device = 0;
     IaParams P;
@@ -31,16 +43,17 @@ struct ia_ctx {
      * slot = [work counter of the bulk kernel, number handed over, work counter of the cooperative kernel, pad] */
     unsigned long long *counters = nullptr;
     unsigned counter_next = 0;
-    IaHand *queue = nullptr; /* hand-over queue: one entry per lane of a full bulk grid */
-    size_t queue_cap = 0;
+    size_t queue_cap = 0; /* entries of one hand-over queue: one per lane of a full bulk grid */
     int handoff_lanes = 16;
     int n_sm = 0;
     IaKernelInfo kinfo[2]; /* 0 bulk, 1 cooperative */
-    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr}; /* start, between the kernels, end of the last run */
-    bool timed = false;
-    /* staging for ia_run_host */
-    void *stage = nullptr;
-    size_t stage_bytes = 0;
+    /* Run slots.  A run occupies slot seq % max(depth, 1): its hand-over queue, the stream its straggler
+     * kernel runs on (depth > 0; with depth 0 it follows the bulk kernel on the caller's stream), the
+     * events around its kernels and, for the host entry points, its device staging. */
+    int depth = 0;
+    unsigned long long seq = 0;
+    IaSlot slot[IA_PIPE_MAX];
+    cudaStream_t host_stream = nullptr; /* ia_submit_host / ia_run_host */
     std::string err;
 };
 
@@ -53,6 +66,19 @@ static int fail_cuda(ia_ctx *c, const char *what, cudaError_t e) {
 static int fail_inval(ia_ctx *c, const char *what) {
     if (c) c->err = what;
     return IA_EINVAL;
+}
+
+/* allocates what slot k owns (idempotent) */
+static cudaError_t slot_init(ia_ctx *c, int k) {
+    IaSlot &s = c->slot[k];
+    cudaError_t e = cudaSuccess;
+    if (!s.queue) e = cudaMalloc(&s.queue, c->queue_cap * sizeof(IaHand));
+    /* default priority, like the caller's stream: the next run's bulk kernel (already queued behind this run's
+     * on the caller's stream) takes the SMs first and the straggler kernel fills in as its blocks drain */
+    if (e == cudaSuccess && !s.tail) e = cudaStreamCreateWithFlags(&s.tail, cudaStreamNonBlocking);
+    for (int j = 0; j < 4 && e == cudaSuccess; ++j)
+        if (!s.ev[j]) e = cudaEventCreate(&s.ev[j]);
+    return e;
 }
 
 extern "C" {
@@ -149,9 +175,9 @@ int ia_create(ia_ctx **out, const ia_species *sp, const ia_trap *tr, double De_K
                                &c->kinfo[k].regs, &c->kinfo[k].local_bytes);
     if (e == cudaSuccess) {
         c->queue_cap = (size_t)c->n_sm * c->kinfo[0].blocks_per_sm * c->kinfo[0].threads_per_block;
-        e = cudaMalloc(&c->queue, c->queue_cap * sizeof(IaHand));
+        e = slot_init(c, 0);
     }
-    for (int k = 0; k < 3 && e == cudaSuccess; ++k) e = cudaEventCreate(&c->ev[k]);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->host_stream, cudaStreamNonBlocking);
     if (e != cudaSuccess) {
         const int rc = e == cudaErrorMemoryAllocation ? IA_ENOMEM : IA_ECUDA;
         ia_destroy(c);
@@ -164,11 +190,20 @@ int ia_create(ia_ctx **out, const ia_species *sp, const ia_trap *tr, double De_K
 int ia_destroy(ia_ctx *ctx) {
     if (!ctx) return IA_EINVAL;
     cudaSetDevice(ctx->device);
+    /* runs still in flight finish first: their kernels use the ctx's scratch */
+    if (ctx->host_stream) cudaStreamSynchronize(ctx->host_stream);
+    for (int k = 0; k < IA_PIPE_MAX; ++k) {
+        IaSlot &s = ctx->slot[k];
+        if (s.used) cudaEventSynchronize(s.ev[2]);
+        if (s.host_used) cudaEventSynchronize(s.ev[3]);
+        if (s.tail) cudaStreamDestroy(s.tail);
+        if (s.queue) cudaFree(s.queue);
+        if (s.stage) cudaFree(s.stage);
+        for (int j = 0; j < 4; ++j)
+            if (s.ev[j]) cudaEventDestroy(s.ev[j]);
+    }
+    if (ctx->host_stream) cudaStreamDestroy(ctx->host_stream);
     if (ctx->counters) cudaFree(ctx->counters);
-    if (ctx->queue) cudaFree(ctx->queue);
-    if (ctx->stage) cudaFree(ctx->stage);
-    for (int k = 0; k < 3; ++k)
-        if (ctx->ev[k]) cudaEventDestroy(ctx->ev[k]);
     delete ctx;
     return IA_OK;
 }
@@ -196,18 +231,51 @@ int ia_set_handoff(ia_ctx *ctx, int lanes) {
     return IA_OK;
 }
 
-int ia_get_last_timing(ia_ctx *ctx, double *bulk_ms, double *coop_ms) {
-    if (!ctx || !bulk_ms || !coop_ms) return IA_EINVAL;
-    if (!ctx->timed) return fail_inval(ctx, "no run has been timed on this ctx yet");
+int ia_set_pipeline(ia_ctx *ctx, int depth) {
+    if (!ctx) return IA_EINVAL;
+    if (depth < 0 || depth > IA_PIPE_MAX) return fail_inval(ctx, "ia_set_pipeline: depth must be in [0, 16]");
     cudaError_t e = cudaSetDevice(ctx->device);
-    if (e == cudaSuccess) e = cudaEventSynchronize(ctx->ev[2]);
+    /* runs in flight keep their slots: let them finish before the slot numbering changes */
+    for (int k = 0; k < IA_PIPE_MAX && e == cudaSuccess; ++k)
+        if (ctx->slot[k].used) e = cudaEventSynchronize(ctx->slot[k].ev[2]);
+    for (int k = 0; k < depth && e == cudaSuccess; ++k) e = slot_init(ctx, k);
+    if (e == cudaErrorMemoryAllocation) {
+        ctx->err = "ia_set_pipeline: hand-over queue allocation failed";
+        return IA_ENOMEM;
+    }
+    if (e != cudaSuccess) return fail_cuda(ctx, "ia_set_pipeline", e);
+    ctx->depth = depth;
+    return IA_OK;
+}
+
+int ia_join(ia_ctx *ctx, void *cuda_stream) {
+    if (!ctx) return IA_EINVAL;
+    cudaError_t e = cudaSetDevice(ctx->device);
+    for (int k = 0; k < IA_PIPE_MAX && e == cudaSuccess; ++k)
+        if (ctx->slot[k].used) e = cudaStreamWaitEvent((cudaStream_t)cuda_stream, ctx->slot[k].ev[2], 0);
+    if (e != cudaSuccess) return fail_cuda(ctx, "ia_join", e);
+    return IA_OK;
+}
+
+int ia_get_timing(ia_ctx *ctx, int runs_back, double *bulk_ms, double *coop_ms) {
+    if (!ctx || !bulk_ms || !coop_ms) return IA_EINVAL;
+    const int ring = ctx->depth > 0 ? ctx->depth : 1;
+    if (runs_back < 0 || runs_back >= ring || (unsigned long long)runs_back >= ctx->seq)
+        return fail_inval(ctx, "ia_get_timing: that run is no longer (or not yet) on record");
+    IaSlot &s = ctx->slot[(ctx->seq - 1 - (unsigned long long)runs_back) % (unsigned long long)ring];
+    cudaError_t e = cudaSetDevice(ctx->device);
+    if (e == cudaSuccess) e = cudaEventSynchronize(s.ev[2]);
     float a = 0.f, b = 0.f;
-    if (e == cudaSuccess) e = cudaEventElapsedTime(&a, ctx->ev[0], ctx->ev[1]);
-    if (e == cudaSuccess) e = cudaEventElapsedTime(&b, ctx->ev[1], ctx->ev[2]);
-    if (e != cudaSuccess) return fail_cuda(ctx, "ia_get_last_timing", e);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&a, s.ev[0], s.ev[1]);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&b, s.ev[1], s.ev[2]);
+    if (e != cudaSuccess) return fail_cuda(ctx, "ia_get_timing", e);
     *bulk_ms = a;
     *coop_ms = b;
     return IA_OK;
+}
+
+int ia_get_last_timing(ia_ctx *ctx, double *bulk_ms, double *coop_ms) {
+    return ia_get_timing(ctx, 0, bulk_ms, coop_ms);
 }
 
 } // extern "C"
@@ -276,10 +344,9 @@ static int grid_for(const ia_ctx *ctx, int k, unsigned long long n) {
     return (int)(need < full ? need : full);
 }
 
-extern "C" {
-
-int ia_run(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *outputs, void *cuda_stream) {
-    if (!ctx) return IA_EINVAL;
+/* ia_run proper; *slot_out receives the run slot (only when something was launched, else -1) */
+static int run_impl(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *outputs, cudaStream_t st, int *slot_out) {
+    *slot_out = -1;
     ctx->err.clear();
     if (!outputs) return fail_inval(ctx, "outputs is NULL");
     IaGen G;
@@ -287,9 +354,16 @@ int ia_run(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *outputs, void
     int rc = make_gen(ctx, launch, &G, &warn);
     if (rc != IA_OK) return rc;
     if (G.n == 0) return IA_OK;
-    cudaStream_t st = (cudaStream_t)cuda_stream;
     cudaError_t e = cudaSetDevice(ctx->device);
     if (e != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", e);
+    const int k = ctx->depth > 0 ? (int)(ctx->seq % (unsigned long long)ctx->depth) : 0;
+    IaSlot &sl = ctx->slot[k];
+    /* the slot's queue and events are free again once the run that used them last has ended; with
+     * depth > 0 that run's straggler kernel is on another stream, so the caller's stream waits for it */
+    if (ctx->depth > 0 && sl.used) {
+        e = cudaStreamWaitEvent(st, sl.ev[2], 0);
+        if (e != cudaSuccess) return fail_cuda(ctx, "cudaStreamWaitEvent(slot)", e);
+    }
     unsigned long long *scratch = ctx->counters + 4 * (size_t)(ctx->counter_next++ % IA_COUNTER_RING);
     e = cudaMemsetAsync(scratch, 0, 4 * sizeof(unsigned long long), st);
     if (e != cudaSuccess) return fail_cuda(ctx, "cudaMemsetAsync(counter)", e);
@@ -303,40 +377,49 @@ int ia_run(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *outputs, void
     std::memset(&S, 0, sizeof(S));
     S.counter = scratch;
     S.warn = warn;
-    e = cudaEventRecord(ctx->ev[0], st);
+    cudaStream_t end_stream = st;
+    e = cudaEventRecord(sl.ev[0], st);
     if (e != cudaSuccess) return fail_cuda(ctx, "cudaEventRecord", e);
     if (coop_only) {
         e = ia_launch_persistent(3, ctx->P, G, O, S, grid_for(ctx, 1, G.n), st);
-        if (e == cudaSuccess) e = cudaEventRecord(ctx->ev[1], st);
+        if (e == cudaSuccess) e = cudaEventRecord(sl.ev[1], st);
     } else {
         if (handoff) {
-            S.q_out = ctx->queue;
+            S.q_out = sl.queue;
             S.n_out = scratch + 1;
             S.handoff_lanes = ctx->handoff_lanes;
         }
         const int blocks = grid_for(ctx, 0, G.n);
         e = ia_launch_persistent(1, ctx->P, G, O, S, blocks, st);
-        if (e == cudaSuccess) e = cudaEventRecord(ctx->ev[1], st);
+        if (e == cudaSuccess) e = cudaEventRecord(sl.ev[1], st);
         if (e == cudaSuccess && handoff) {
-            /* the straggler kernel resumes what the bulk kernel queued; it is enqueued behind it on the same
-             * stream with a grid that can hold every lane the bulk grid could have handed over */
+            /* the straggler kernel resumes what the bulk kernel queued, with a grid that can hold every lane
+             * the bulk grid could have handed over.  depth 0: behind the bulk kernel on the caller's stream.
+             * depth > 0: on the slot's own stream, so that the caller's stream is free for the next run's bulk
+             * kernel while this run's longest trajectories finish. */
             IaSched S5;
             std::memset(&S5, 0, sizeof(S5));
             S5.counter = scratch + 2;
-            S5.q_in = ctx->queue;
+            S5.q_in = sl.queue;
             S5.n_in = scratch + 1;
+            if (ctx->depth > 0) {
+                end_stream = sl.tail;
+                e = cudaStreamWaitEvent(end_stream, sl.ev[1], 0);
+            }
             const unsigned long long most = (unsigned long long)blocks * (unsigned long long)ctx->handoff_lanes;
-            e = ia_launch_persistent(3, ctx->P, G, O, S5, grid_for(ctx, 1, most), st);
+            if (e == cudaSuccess) e = ia_launch_persistent(3, ctx->P, G, O, S5, grid_for(ctx, 1, most), end_stream);
         }
     }
-    if (e == cudaSuccess) e = cudaEventRecord(ctx->ev[2], st);
+    if (e == cudaSuccess) e = cudaEventRecord(sl.ev[2], end_stream);
     if (e != cudaSuccess) return fail_cuda(ctx, "persistent kernel launch", e);
-    ctx->timed = true;
+    sl.used = true;
+    ctx->seq++;
+    *slot_out = k;
     return IA_OK;
 }
 
-int ia_run_host(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *host_out) {
-    if (!ctx) return IA_EINVAL;
+/* enqueues one host-buffer run: H2D, kernels, D2H; nothing here waits for the device */
+static int submit_host_impl(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *host_out) {
     ctx->err.clear();
     if (!launch || !host_out) return fail_inval(ctx, "launch or outputs is NULL");
     const uint64_t n = launch->n;
@@ -345,30 +428,37 @@ int ia_run_host(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *host_out
         return fail_inval(ctx, "EXPLICIT launch needs y0 and phase");
     cudaError_t e = cudaSetDevice(ctx->device);
     if (e != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", e);
+    const int k = ctx->depth > 0 ? (int)(ctx->seq % (unsigned long long)ctx->depth) : 0;
+    IaSlot &sl = ctx->slot[k];
+    cudaStream_t st = ctx->host_stream;
     /* staging layout: [summary 512][records n*64][ic_dump n*14*8][y0 n*12*8][phase n*8] */
     const size_t off_rec = sizeof(ia_summary);
     const size_t off_ic = off_rec + (host_out->records ? n * sizeof(ia_record) : 0);
     const size_t off_y0 = off_ic + (host_out->ic_dump ? n * 14 * sizeof(double) : 0);
     const size_t off_ph = off_y0 + (launch->mode == IA_IC_EXPLICIT ? n * 12 * sizeof(double) : 0);
     const size_t total = off_ph + (launch->mode == IA_IC_EXPLICIT ? n * sizeof(double) : 0);
-    if (total > ctx->stage_bytes) {
-        if (ctx->stage) cudaFree(ctx->stage);
-        ctx->stage = nullptr;
-        ctx->stage_bytes = 0;
-        e = cudaMalloc(&ctx->stage, total);
+    if (total > sl.stage_bytes) {
+        if (sl.host_used) cudaEventSynchronize(sl.ev[3]); /* the slot's previous run still copies from it */
+        if (sl.stage) cudaFree(sl.stage);
+        sl.stage = nullptr;
+        sl.stage_bytes = 0;
+        e = cudaMalloc(&sl.stage, total);
         if (e != cudaSuccess) {
             ctx->err = "device staging allocation failed";
             return IA_ENOMEM;
         }
-        ctx->stage_bytes = total;
+        sl.stage_bytes = total;
     }
-    char *base = (char *)ctx->stage;
+    if (sl.host_used) { /* the staging is free again once the slot's previous copies back are done */
+        e = cudaStreamWaitEvent(st, sl.ev[3], 0);
+        if (e != cudaSuccess) return fail_cuda(ctx, "cudaStreamWaitEvent(staging)", e);
+    }
+    char *base = (char *)sl.stage;
     ia_launch L = *launch;
     ia_outputs O;
     O.summary = (ia_summary *)base;
     O.records = host_out->records ? (ia_record *)(base + off_rec) : nullptr;
     O.ic_dump = host_out->ic_dump ? (double *)(base + off_ic) : nullptr;
-    cudaStream_t st = 0;
     e = cudaMemsetAsync(base, 0, sizeof(ia_summary), st);
     if (e != cudaSuccess) return fail_cuda(ctx, "cudaMemsetAsync(summary)", e);
     if (launch->mode == IA_IC_EXPLICIT) {
@@ -379,19 +469,59 @@ int ia_run_host(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *host_out
         L.y0 = (const double *)(base + off_y0);
         L.phase = (const double *)(base + off_ph);
     }
-    int rc = ia_run(ctx, &L, &O, st);
+    int used = -1;
+    int rc = run_impl(ctx, &L, &O, st, &used);
     if (rc != IA_OK) return rc;
     const std::string warn_text = ctx->err;
+    /* the copies back follow the run's last kernel: on the slot's straggler stream when there is one */
+    cudaStream_t back = st;
+    if (ctx->depth > 0 && launch->path == IA_PATH_AUTO && ctx->handoff_lanes > 0) back = sl.tail;
     if (host_out->records)
-        e = cudaMemcpyAsync(host_out->records, O.records, n * sizeof(ia_record), cudaMemcpyDeviceToHost, st);
+        e = cudaMemcpyAsync(host_out->records, O.records, n * sizeof(ia_record), cudaMemcpyDeviceToHost, back);
     if (e == cudaSuccess && host_out->ic_dump)
-        e = cudaMemcpyAsync(host_out->ic_dump, O.ic_dump, n * 14 * sizeof(double), cudaMemcpyDeviceToHost, st);
+        e = cudaMemcpyAsync(host_out->ic_dump, O.ic_dump, n * 14 * sizeof(double), cudaMemcpyDeviceToHost, back);
     if (e == cudaSuccess && host_out->summary)
-        e = cudaMemcpyAsync(host_out->summary, O.summary, sizeof(ia_summary), cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    if (e != cudaSuccess) return fail_cuda(ctx, "D2H copy / synchronise", e);
+        e = cudaMemcpyAsync(host_out->summary, O.summary, sizeof(ia_summary), cudaMemcpyDeviceToHost, back);
+    if (e == cudaSuccess) e = cudaEventRecord(sl.ev[3], back);
+    if (e != cudaSuccess) return fail_cuda(ctx, "D2H copy", e);
+    sl.host_used = true;
     ctx->err = warn_text;
     return IA_OK;
+}
+
+extern "C" {
+
+int ia_run(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *outputs, void *cuda_stream) {
+    if (!ctx) return IA_EINVAL;
+    int slot;
+    return run_impl(ctx, launch, outputs, (cudaStream_t)cuda_stream, &slot);
+}
+
+int ia_submit_host(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *host_outputs) {
+    if (!ctx) return IA_EINVAL;
+    return submit_host_impl(ctx, launch, host_outputs);
+}
+
+int ia_wait(ia_ctx *ctx) {
+    if (!ctx) return IA_EINVAL;
+    cudaError_t e = cudaSetDevice(ctx->device);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->host_stream);
+    for (int k = 0; k < IA_PIPE_MAX && e == cudaSuccess; ++k) {
+        if (ctx->slot[k].used) e = cudaEventSynchronize(ctx->slot[k].ev[2]);
+        if (e == cudaSuccess && ctx->slot[k].host_used) e = cudaEventSynchronize(ctx->slot[k].ev[3]);
+    }
+    if (e != cudaSuccess) return fail_cuda(ctx, "ia_wait", e);
+    return IA_OK;
+}
+
+int ia_run_host(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *host_outputs) {
+    if (!ctx) return IA_EINVAL;
+    int rc = submit_host_impl(ctx, launch, host_outputs);
+    if (rc != IA_OK) return rc;
+    const std::string warn_text = ctx->err;
+    rc = ia_wait(ctx);
+    if (rc == IA_OK) ctx->err = warn_text;
+    return rc;
 }
 
 int ia_generate(ia_ctx *ctx, const ia_launch *launch, double *ic_dump, void *cuda_stream) {

@@ -110,30 +110,39 @@ IA_DEV double ia_rcp(double x) {
     return fma(y, e2, y);
 }
 
-/* x^(-1/5) for x in [1e-30, 1e30]: FP32 MUFU seed (lg2/ex2, rel. err ~1e-6) and two Newton steps
- * y <- y (6 - x y^5)/5 (rel. err -> 3e-12 -> ~3e-23). */
+/* x^(-1/5) for x in [1e-30, 1e30]: FP32 MUFU seed (lg2/ex2, rel. err ~1e-6) and one Newton step
+ * y <- y (6 - x y^5)/5 (rel. err -> 3 e^2 ~ 3e-12).  The result only scales the next step size: a relative
+ * 3e-12 there moves the next step's error estimate by 1.5e-11 of itself, far below its own rounding. */
 IA_DEV double ia_inv_fifth_root(double x) {
     const float xf = (float)x;
     float lf;
     asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(lf) : "f"(xf));
     float sf;
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(sf) : "f"(-0.2f * lf));
-    double y = (double)sf;
-#pragma unroll
-    for (int it = 0; it < 2; ++it) {
-        const double y2 = y * y;
-        const double y4 = y2 * y2;
-        const double y5 = y4 * y;
-        const double t = fma(-x, y5, 6.0);
-        y = (0.2 * y) * t;
-    }
-    return y;
+    const double y = (double)sf;
+    const double y2 = y * y;
+    const double y4 = y2 * y2;
+    const double y5 = y4 * y;
+    const double t = fma(-x, y5, 6.0);
+    return (0.2 * y) * t;
 }
 
 /* cos(arg) for arg in about [-4 pi, 8 pi] (the callers keep time folded, reading R9):
  * n = rint(arg/pi), r = arg - n pi (two-constant Cody-Waite with exact fma products),
- * cos(arg) = (-1)^n cos(r), |r| <= pi/2, Taylor polynomial in z = r^2 through r^22
- * (truncation (pi/2)^24/24! = 8e-20; absolute error ~1e-16). */
+ * cos(arg) = (-1)^n cos(r), |r| <= pi/2.  cos(r) is a degree-8 polynomial in z = r^2, the minimax fit
+ * (Remez, absolute error, 60-digit arithmetic) on |r| <= 1.0001 pi/2: 3.9e-18 before and 4.4e-17 after
+ * rounding the coefficients to double -- below half an ulp of 1, so the polynomial's own error is hidden
+ * by the ~1e-16 rounding of the Horner chain (the Taylor series needs three more terms for that).
+ * tests/test_host_logic.py re-evaluates these literals against a 50-digit cosine. */
+#define IA_COS_C8 (+4.60897384029083775838e-14)
+#define IA_COS_C7 (-1.14629017962301774571e-11)
+#define IA_COS_C6 (+2.08765618439870221873e-09)
+#define IA_COS_C5 (-2.75573163912833653934e-07)
+#define IA_COS_C4 (+2.48015872774199032044e-05)
+#define IA_COS_C3 (-1.38888888887730337432e-03)
+#define IA_COS_C2 (+4.16666666666638818572e-02)
+#define IA_COS_C1 (-4.99999999999999722444e-01)
+#define IA_COS_C0 (+1.00000000000000000000e+00)
 IA_DEV double ia_cos_folded(double arg) {
     const double MAGIC = 6755399441055744.0; /* 1.5 * 2^52: adding it rounds to nearest integer */
     const double nf = fma(arg, 0.31830988618379067154, MAGIC);
@@ -141,23 +150,27 @@ IA_DEV double ia_cos_folded(double arg) {
     double r = fma(-n, 3.14159265358979311600e+00, arg);
     r = fma(-n, 1.22464679914735317723e-16, r);
     const double z = r * r;
-    double p = -1.0 / 1124000727777607680000.0;         /* -1/22! */
-    p = fma(p, z, 1.0 / 2432902008176640000.0);         /*  1/20! */
-    p = fma(p, z, -1.0 / 6402373705728000.0);           /* -1/18! */
-    p = fma(p, z, 1.0 / 20922789888000.0);              /*  1/16! */
-    p = fma(p, z, -1.0 / 87178291200.0);                /* -1/14! */
-    p = fma(p, z, 1.0 / 479001600.0);                   /*  1/12! */
-    p = fma(p, z, -1.0 / 3628800.0);                    /* -1/10! */
-    p = fma(p, z, 1.0 / 40320.0);                       /*  1/8!  */
-    p = fma(p, z, -1.0 / 720.0);                        /* -1/6!  */
-    p = fma(p, z, 1.0 / 24.0);                          /*  1/4!  */
-    p = fma(p, z, -0.5);                                /* -1/2!  */
-    p = fma(p, z, 1.0);
+    double p = IA_COS_C8;
+    p = fma(p, z, IA_COS_C7);
+    p = fma(p, z, IA_COS_C6);
+    p = fma(p, z, IA_COS_C5);
+    p = fma(p, z, IA_COS_C4);
+    p = fma(p, z, IA_COS_C3);
+    p = fma(p, z, IA_COS_C2);
+    p = fma(p, z, IA_COS_C1);
+    p = fma(p, z, IA_COS_C0);
     /* flip the sign when n is odd: the integer n sits in the low word of nf */
     const int lo = __double2loint(nf);
     const int hi = __double2hiint(p) ^ (lo << 31);
     return __hiloint2double(hi, __double2loint(p));
 }
+
+/* max / min by one comparison and a select (DSETP + 2 FSEL).  The library fmax/fmin cost twice that on
+ * sm_100a (NaN canonicalisation and register shuffling around DSETP.MAX).  Semantics with a NaN operand:
+ * the comparison is false, so ia_max(a, b) and ia_min(a, b) return b -- every caller states which operand
+ * may be NaN. */
+IA_DEV double ia_max(double a, double b) { return a > b ? a : b; }
+IA_DEV double ia_min(double a, double b) { return a < b ? a : b; }
 
 /* Scheduling fence without an instruction: makes `x` look redefined once `after` is known, so that the
  * chain starting from x is not hoisted above the computation of `after` (register pressure only). */
@@ -251,9 +264,15 @@ struct IaErr {
     double num, den; /* err = num/den = max_i |e_i| / max(|y_i|, |ynew_i|, thr) */
 };
 
-/* keeps the larger of two ratios na/da, nb/db (all >= 0, denominators > 0) by cross-multiplication */
+/* Magnitudes are never materialised in the norm: the operands keep their sign and every use takes |.|,
+ * which is an operand modifier of DSETP / DMUL / FSEL (a separate fabs costs a DADD on the FP64 pipe). */
+
+/* the operand of larger magnitude, sign kept (b when they are equal or a is NaN) */
+IA_DEV double ia_absmax_raw(double a, double b) { return fabs(a) > fabs(b) ? a : b; }
+
+/* keeps the larger of two ratios |na|/|da|, |nb|/|db| (denominators non-zero) by cross-multiplication */
 IA_DEV void ia_ratio_max(double &na, double &da, double nb, double db) {
-    const bool gt = nb * da > na * db;
+    const bool gt = fabs(nb) * fabs(da) > fabs(na) * fabs(db);
     na = gt ? nb : na;
     da = gt ? db : da;
 }
@@ -382,10 +401,10 @@ IA_DEV void ia_dp5_attempt(const IaParams &P, const IaLane<LPT> &L, const IaVec<
         for (int a = 0; a < NA; ++a) {
             const double fvi = IA_F(p7, N.Ai[a], evi[a]);
             const double fva = IA_F(p7, N.Aa[a], eva[a]);
-            double n_i = fabs(exi[a]), d_i = fmax(fmax(fabs(Y.xi[a]), fabs(N.xi[a])), P.thr);
-            ia_ratio_max(n_i, d_i, fabs(fvi), fmax(fmax(fabs(Y.vi[a]), fabs(N.vi[a])), P.thr));
-            double n_a = fabs(exa[a]), d_a = fmax(fmax(fabs(Y.xa[a]), fabs(N.xa[a])), P.thr);
-            ia_ratio_max(n_a, d_a, fabs(fva), fmax(fmax(fabs(Y.va[a]), fabs(N.va[a])), P.thr));
+            double n_i = exi[a], d_i = ia_absmax_raw(ia_absmax_raw(Y.xi[a], N.xi[a]), P.thr);
+            ia_ratio_max(n_i, d_i, fvi, ia_absmax_raw(ia_absmax_raw(Y.vi[a], N.vi[a]), P.thr));
+            double n_a = exa[a], d_a = ia_absmax_raw(ia_absmax_raw(Y.xa[a], N.xa[a]), P.thr);
+            ia_ratio_max(n_a, d_a, fva, ia_absmax_raw(ia_absmax_raw(Y.va[a], N.va[a]), P.thr));
             ia_ratio_max(n_i, d_i, n_a, d_a);
             en[a] = n_i;
             sc[a] = d_i;
@@ -395,8 +414,8 @@ IA_DEV void ia_dp5_attempt(const IaParams &P, const IaLane<LPT> &L, const IaVec<
         ia_gather3<LPT>(L, sc, SC);
         ia_ratio_max(EN[0], SC[0], EN[1], SC[1]);
         ia_ratio_max(EN[0], SC[0], EN[2], SC[2]);
-        out.err.num = EN[0];
-        out.err.den = SC[0];
+        out.err.num = fabs(EN[0]);
+        out.err.den = fabs(SC[0]);
     }
 #undef IA_F
 }

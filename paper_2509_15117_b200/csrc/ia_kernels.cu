@@ -336,7 +336,7 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
         const bool accept = so.finite && (so.err.num <= P.rtol * so.err.den);
         double xr = so.err.num * ia_rcp(so.err.den * P.rtol); /* err / rtol */
         xr = so.finite ? xr : 1e30;
-        xr = fmax(fmin(xr, 1e30), 1e-30); /* NaN -> 1e30 (fmin returns the non-NaN operand) */
+        xr = ia_max(ia_min(xr, 1e30), 1e-30); /* NaN -> 1e30 (ia_min returns its second operand then) */
         const double fac = 0.8 * ia_inv_fifth_root(xr); /* 0.8 (rtol/err)^(1/5) */
         const double now = (double)n_per * P.T_rf + tf;
         const double g = so.r2n - P.r0sq;
@@ -388,8 +388,8 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
         }
         /* step size of the next attempt (R5) */
         {
-            const double h_acc = fmin(failed ? hs : hs * fmin(5.0, fac), P.h_max);
-            const double h_rej = fmax(P.h_min, failed ? 0.5 * hs : hs * fmax(0.1, fac));
+            const double h_acc = ia_min(failed ? hs : hs * ia_min(fac, 5.0), P.h_max);
+            const double h_rej = ia_max(failed ? 0.5 * hs : hs * ia_max(fac, 0.1), P.h_min);
             h = commit ? h_acc : (rej ? h_rej : hs);
             failed = commit ? false : (rej ? true : failed);
         }

@@ -230,6 +230,52 @@ def test_bulk_coop_and_handoff_paths_are_bit_identical(P, which):
     assert np.array_equal(s_bulk["hist_ncoll"], s_coop["hist_ncoll"])
 
 
+def test_pipelined_runs_match_serial_runs(P):
+    """ia_set_pipeline(3): five runs enqueued back to back (straggler kernels on the library's own streams,
+    runs 4 and 5 recycling the slots of runs 1 and 2), joined once, give the records and summaries of the same
+    five runs done one after the other; the same through ia_submit_host / ia_wait with host buffers."""
+    import torch
+    cell = I.config1(40)
+    cell = replace(cell, params=replace(cell.params, t_max_rf=200.0))
+    n = cell.launch.n
+    launches = [replace(cell.launch, phase0=0.3 * k) for k in range(5)]
+    with P.Context(cell.params) as ctx:
+        ctx.set_handoff(32)
+        serial = [ctx.run_sync(L)[:2] for L in launches]
+        ctx.set_pipeline(3)
+        bufs = [ctx.alloc(n) for _ in launches]
+        for L, (rec, summ, _) in zip(launches, bufs):
+            ctx.run(L, records=rec, summary=summ)
+        ctx.join()
+        torch.cuda.synchronize()
+        for (rec, summ, _), (rec0, summ0) in zip(bufs, serial):
+            _assert_records_identical(P.view_records(rec, n), rec0)
+            s = P.view_summary(summ)
+            for f in ("n_done", "n_complex", "steps_acc", "steps_rej", "steps_loc", "n_handoff", "steps_coop"):
+                assert int(s[f]) == int(summ0[f]), f
+        assert int(serial[0][1]["n_handoff"]) > 0
+        t = [ctx.timing(back) for back in range(3)]
+        assert all(x["bulk_ms"] > 0.0 and x["coop_ms"] > 0.0 for x in t)
+        with pytest.raises(P.IaError):
+            ctx.timing(3)
+        # host entry points, asynchronous form
+        ic = ctx.generate(launches[1])
+        y0 = torch.from_numpy(np.ascontiguousarray(ic[:, :12])).pin_memory()
+        ph = torch.from_numpy(np.ascontiguousarray(ic[:, 12])).pin_memory()
+        cl = P.make_launch(I.Launch(mode=I.MODE_EXPLICIT, n=n), y0, ph)
+        host = [(torch.zeros(n * P.RECORD_BYTES, dtype=torch.uint8).pin_memory(),
+                 torch.zeros(P.SUMMARY_BYTES, dtype=torch.uint8).pin_memory()) for _ in range(4)]
+        for rec_h, sum_h in host:
+            P.ia_submit_host(ctx.handle, cl, rec_h, sum_h)
+        ctx.wait()
+        for rec_h, sum_h in host:
+            _assert_records_identical(rec_h.numpy().view(P.RECORD_DTYPE), serial[1][0])
+            assert int(sum_h.numpy().view(P.SUMMARY_DTYPE)[0]["n_done"]) == n
+        ctx.set_pipeline(0)
+        rec1, _ = ctx.run_sync(launches[2])[:2]
+        _assert_records_identical(rec1, serial[2][0])
+
+
 # ---------------------------------------------------------------------------------------------
 # adaptive mode, non-chaotic: config 0 in full (north_star: final observables to a relative 1e-8; R15)
 # ---------------------------------------------------------------------------------------------
