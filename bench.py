@@ -46,7 +46,7 @@ ORACLE_SAMPLE_EVERY = 8   # cpu_baseline: every 8th grid point in theta and phi 
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=8)
+    ap.add_argument("--steps", type=int, default=16)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--n-side", type=int, default=512)
@@ -60,9 +60,11 @@ def parse():
     ap.add_argument("--handoff", type=int, default=-1,
                     help="hand-over threshold of the bulk kernel in lanes (0 = bulk kernel only; default: the library's)")
     ap.add_argument("--path", type=int, default=0, help="ia_path: 0 production kernel pair, 1 bulk only, 2 cooperative only")
-    ap.add_argument("--pipeline", type=int, default=16,
-                    help="ia_set_pipeline depth: how many passes may still be finishing their longest trajectories on "
-                         "the library's straggler streams while later passes start (0 = strictly one pass after another)")
+    ap.add_argument("--pipeline", type=int, default=64,
+                    help="ia_set_pipeline depth: passes per generation, i.e. how many passes share one straggler kernel "
+                         "(it runs on the library's stream while the next generation's bulk kernels run); "
+                         "0 = strictly one pass after another, both kernels of a pass back to back")
+    ap.add_argument("--chain", default="", help="levels,budget of the straggler chain (ia_set_chain); default: the library's")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -236,11 +238,15 @@ def run_ours(args):
     ctx = P.Context(cell.params, device=local)
     if args.handoff >= 0:
         ctx.set_handoff(args.handoff)
-    depth = max(0, min(args.pipeline, 16))
+    levels = P.IA_STRAGGLER_LEVELS
+    if args.chain:
+        levels, budget = (int(x) for x in args.chain.split(","))
+        ctx.set_chain(levels, budget)
+    depth = max(0, min(args.pipeline, 64, K))
     ctx.set_pipeline(depth)
     launch = dataclasses.replace(launch, path=args.path)
     info = ctx.kernel_info
-    nbuf = min(K, max(depth, 1))                 # passes in flight never share an output buffer
+    nbuf = min(K, 2 * max(depth, 1))             # passes in flight (two generations) never share an output buffer
     recs_d = [torch.empty(n * P.RECORD_BYTES, dtype=torch.uint8, device=dev) for _ in range(nbuf)]
     summaries = torch.zeros((W + K, P.SUMMARY_BYTES), dtype=torch.uint8, device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
@@ -255,8 +261,9 @@ def run_ours(args):
     clocks.start()
     ev0.record()
     for k in range(K):
-        # one step = one pass over the grid = bulk kernel + straggler kernel (the latter on the library's
-        # own stream when depth > 0, so that pass k+1 starts while pass k's longest trajectories finish)
+        # one step = one pass over the grid: its bulk kernel here; its stragglers are finished by the straggler
+        # kernel of its generation (depth 0: right behind the bulk kernel; depth > 0: one launch for `depth` passes,
+        # on the library's stream, while the next generation's bulk kernels run)
         ctx.run(launch, records=recs_d[k % nbuf], summary=summaries[W + k])
         flush.fill_(k)                                             # L2 flush between timed iterations
     ctx.join()                                                     # the stream waits for every straggler kernel
@@ -264,7 +271,13 @@ def run_ours(args):
     barrier()
     clk = clocks.stop()
     total_s = D.all_reduce_max(ev0.elapsed_time(ev1) * 1e-3, dev)
-    kernel_times = [ctx.timing(back) for back in range(min(K, max(depth, 1)))]   # the library's own CUDA events
+    kernel_times = []                              # the library's own CUDA events around each kernel
+    for back in range(K):
+        try:
+            kernel_times.append(ctx.timing(back))
+        except P.IaError:                          # older than the two generations the library keeps on record
+            break
+    n_coop_launches = K if depth == 0 else -(-K // depth)
     summ = P.view_summary(summaries[W + K - 1])
     bulk_ms = float(np.mean([t["bulk_ms"] for t in kernel_times]))
     coop_ms = float(np.mean([t["coop_ms"] for t in kernel_times]))
@@ -330,12 +343,15 @@ def run_ours(args):
                      "share_of_step_time": bulk_ms / step_avg_ms, "share_of_step_flops": 1.0 - steps_coop / max(attempted, 1),
                      "ms_until_work_counter_empty": (int(summ["t_first_idle_ns"]) - int(summ["t_start_ns"])) * 1e-6},
         # the straggler kernel is bound by the serial latency of the longest trajectories, not by throughput
-        "tail": {"kernel": "ia_persistent_kernel<3> (cooperative, 3 lanes per trajectory)", "kernel_ms": coop_ms,
-                 "share_of_step_time": coop_ms / step_avg_ms, "trajectories_handed_over": int(summ["n_handoff"]),
-                 "steps_in_kernel": steps_coop, "longest_trajectory_steps": longest,
+        "tail": {"kernel": f"ia_persistent_kernel<3> (cooperative, 3 lanes per trajectory), chain of {levels} launches",
+                 "kernel_ms": coop_ms,
+                 "launches": n_coop_launches, "passes_per_launch": K / n_coop_launches,
+                 "share_of_step_time": coop_ms * n_coop_launches / K / step_avg_ms,
+                 "trajectories_handed_over_per_pass": int(summ["n_handoff"]),
+                 "steps_in_kernel_per_pass": steps_coop, "longest_trajectory_steps": longest,
                  "us_per_step_serial_bound": 1e3 * coop_ms / max(longest, 1),
                  "note": "a trajectory is a serial chain: the launch cannot end before its longest one (DESIGN.md 'Tail')"},
-        "kernel_info": info, "clocks": clk, "e2e": e2e, "gpu_launches": 2 * K,
+        "kernel_info": info, "clocks": clk, "e2e": e2e, "gpu_launches": K + n_coop_launches * levels,
     }
     if not args.no_cpu_baseline and world == 1:
         s = oracle_sample(cell, args.n_side)

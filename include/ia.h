@@ -80,6 +80,10 @@ typedef enum {
     IA_IC_PHILOX = 2    /* Philox4x32-10(seed; index, cell) directions / phases / energies (R2)     */
 } ia_ic_mode;
 
+/* Launches of the cooperative kernel per straggler phase: a chain of levels, each lasting twice as long
+ * as the one before and re-packing what that one had left ten trajectories to a warp. */
+#define IA_STRAGGLER_LEVELS 12
+
 /* Which kernels propagate a launch.  The bulk kernel runs one lane per trajectory; once the work
  * counter is empty and a warp is down to a few running lanes (ia_set_handoff) it hands them to the
  * cooperative kernel (three lanes per trajectory, a third of the FP64 instructions per lane and
@@ -166,22 +170,24 @@ int ia_run_host(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *host_out
 
 /* Pipelining of successive runs.  Trajectory lengths are power-law distributed
  * (PAPER.md:40): the last few trajectories of a launch take 10^3 times longer than the median, and a
- * trajectory is a serial chain.  With depth d > 0 (at most 16) the straggler kernel of a run goes to a
- * ctx-owned stream, so the caller's stream is free for the bulk kernel of the next run
- * while up to d earlier runs finish their longest trajectories; run number d+1 waits (on the device)
- * for the oldest one.  depth 0 (the default) keeps both kernels on the caller's stream.
- * With depth > 0 the outputs of ia_run are valid only after ia_join: it makes `cuda_stream` wait, on
- * the device, for every straggler kernel enqueued so far (the host does not block).
- * ia_set_pipeline synchronises with the runs in flight; it allocates d hand-over queues (IA_ENOMEM).
- * Streams sharing a hardware work queue serialise: for d > 6 start the process with
- * CUDA_DEVICE_MAX_CONNECTIONS >= d + 2 in its environment (the CUDA default is 8). */
+ * trajectory is a serial chain, so the straggler kernel of a run outlasts its bulk kernel by far.
+ * With depth d > 0 (at most 64) runs are grouped into generations of d: ia_run enqueues only the bulk
+ * kernel, whose hand-overs go to a queue the generation shares; after the d-th run (or at ia_join) ONE
+ * straggler kernel finishes the hand-overs of the whole generation, on a ctx-owned stream, so that the
+ * caller's stream goes on with the bulk kernels of the next generation meanwhile (two generation
+ * buffers; the third generation waits, on the device, for the first).  Each queue entry carries the
+ * outputs of its own run.  depth 0 (the default) keeps both kernels of every run on the caller's stream.
+ * With depth > 0 the outputs of ia_run are valid only after ia_join: it enqueues the straggler kernel of
+ * an incomplete generation and makes `cuda_stream` wait, on the device, for every straggler kernel
+ * enqueued so far (the host does not block).  The runs of one generation must be enqueued on one stream.
+ * ia_set_pipeline synchronises with the runs in flight; it allocates the queues (IA_ENOMEM). */
 int ia_set_pipeline(ia_ctx *ctx, int depth);
 int ia_join(ia_ctx *ctx, void *cuda_stream);
 
 /* Asynchronous form of ia_run_host: enqueues the copies in, the kernels and the copies back on
  * ctx-owned streams and returns; host buffers must be page-locked for the copies to overlap and stay
  * untouched until ia_wait, which blocks the host until every run submitted on this ctx (either way)
- * has finished.  With ia_set_pipeline(d) up to d submitted runs overlap. */
+ * has finished.  With ia_set_pipeline(d) the submitted runs form generations as above. */
 int ia_submit_host(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *host_outputs);
 int ia_wait(ia_ctx *ctx);
 
@@ -223,12 +229,19 @@ int ia_get_kernel_info(const ia_ctx *ctx, int kernel, int *warps_per_sm, int *n_
  * is 16: the cooperative kernel with ten trajectories per warp does the work of ~18 bulk lanes). */
 int ia_set_handoff(ia_ctx *ctx, int lanes);
 
-/* Device times of a run of this ctx, from CUDA events the library records on the launch streams
- * around its kernels: bulk kernel (start -> its end) and cooperative kernel (end of the bulk kernel ->
- * its end, which with a pipeline includes any wait for free SMs), in ms.  runs_back = 0 is the most
- * recent run, 1 the one before ...; only the last max(depth, 1) runs are on record (IA_EINVAL
- * otherwise).  Synchronises with the end of that run.  Host pointers.
- * ia_get_last_timing(ctx, ...) = ia_get_timing(ctx, 0, ...). */
+/* The straggler chain: the cooperative kernel is launched `levels` times in a row
+ * (1..IA_STRAGGLER_LEVELS, the default).  Level j = 0, 1, ... runs until its queue is empty and then for
+ * budget << j further iterations per warp (default 8192, at least 64); what still runs then goes to the
+ * next level, which packs it ten trajectories to a warp again.  The last level keeps everything.
+ * levels = 1: one launch finishes all stragglers.  Applies to the straggler phases enqueued afterwards. */
+int ia_set_chain(ia_ctx *ctx, int levels, uint32_t budget);
+
+/* Device times of a run of this ctx, from CUDA events the library records around its kernels: the run's
+ * bulk kernel, and the straggler kernel that finished its hand-overs (with a pipeline that kernel is
+ * shared by the runs of a generation), in ms.  runs_back = 0 is the most recent run, 1 the one before
+ * ...; a run is on record until its generation buffer is used again (depth 0: the latest run only) and
+ * once its straggler kernel has been enqueued (IA_EINVAL otherwise).  Synchronises with the end of that
+ * run.  Host pointers.  ia_get_last_timing(ctx, ...) = ia_get_timing(ctx, 0, ...). */
 int ia_get_timing(ia_ctx *ctx, int runs_back, double *bulk_ms, double *coop_ms);
 int ia_get_last_timing(ia_ctx *ctx, double *bulk_ms, double *coop_ms);
 

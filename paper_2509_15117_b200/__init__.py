@@ -32,10 +32,11 @@ IA_IC_EXPLICIT, IA_IC_GRID, IA_IC_PHILOX = 0, 1, 2
 IA_PATH_AUTO, IA_PATH_BULK_ONLY, IA_PATH_COOP_ONLY = 0, 1, 2
 IA_ARITH_NOFMA, IA_ARITH_FMA, IA_ARITH_FMA_COOP = 0, 1, 2
 IA_HIST_BINS = 32
+IA_STRAGGLER_LEVELS = 12
 
 # every symbol include/ia.h declares (tests/test_cabi.py checks the library exports each of them)
 EXPORTS = ("ia_create", "ia_run", "ia_run_host", "ia_generate", "ia_step_map", "ia_trace", "ia_get_derived",
-           "ia_get_kernel_info", "ia_set_handoff", "ia_get_last_timing", "ia_get_timing", "ia_set_pipeline", "ia_join",
+           "ia_get_kernel_info", "ia_set_handoff", "ia_set_chain", "ia_get_last_timing", "ia_get_timing", "ia_set_pipeline", "ia_join",
            "ia_submit_host", "ia_wait", "ia_fp64_peak", "ia_destroy", "ia_strerror", "ia_last_error")
 
 
@@ -113,6 +114,7 @@ def load() -> C.CDLL:
     L.ia_get_kernel_info.argtypes = [vp, C.c_int, ip, ip, ip, ip]
     L.ia_set_handoff.argtypes = [vp, C.c_int]
     L.ia_get_last_timing.argtypes = [vp, dp, dp]
+    L.ia_set_chain.argtypes = [vp, C.c_int, C.c_uint32]
     L.ia_get_timing.argtypes = [vp, C.c_int, dp, dp]
     L.ia_set_pipeline.argtypes = [vp, C.c_int]
     L.ia_join.argtypes = [vp, vp]
@@ -250,6 +252,11 @@ def ia_set_handoff(handle, lanes: int) -> None:
     _check(load().ia_set_handoff(handle, int(lanes)), handle)
 
 
+def ia_set_chain(handle, levels: int, budget: int = 8192) -> None:
+    """Straggler chain: `levels` launches of the cooperative kernel, level j lasting budget << j iterations."""
+    _check(load().ia_set_chain(handle, int(levels), int(budget)), handle)
+
+
 def ia_get_timing(handle, runs_back: int = 0) -> dict:
     """Device times (ms) of the two kernels of a recent run on this ctx (0 = the last); synchronises with it."""
     a, b = C.c_double(), C.c_double()
@@ -338,6 +345,9 @@ class Context:
 
     def timing(self, runs_back: int = 0) -> dict:
         return ia_get_timing(self.handle, runs_back)
+
+    def set_chain(self, levels: int, budget: int = 8192) -> None:
+        ia_set_chain(self.handle, levels, budget)
 
     def set_pipeline(self, depth: int) -> None:
         ia_set_pipeline(self.handle, depth)

@@ -23,16 +23,51 @@ struct IaKernelInfo {
     int blocks_per_sm = 0, threads_per_block = 0, regs = 0, local_bytes = 0;
 };
 
-#define IA_PIPE_MAX 16
+#define IA_PIPE_MAX 64     /* runs per generation */
+#define IA_RUN_RING 128    /* runs whose kernel events are kept for ia_get_timing */
+#define IA_COUNTER_RING 256 /* slots of 4 x u64 */
+#define IA_SCRATCH_WORDS 32
 
-struct IaSlot {
-    IaHand *queue = nullptr;
-    cudaStream_t tail = nullptr;             /* non-blocking stream of the straggler kernel               */
-    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr}; /* start, bulk end, run end, host copies done */
-    bool used = false;                       /* ev[2] has been recorded                                    */
-    bool host_used = false;                  /* ev[3] has been recorded                                    */
-    void *stage = nullptr;                   /* device staging of the host entry points                    */
-    size_t stage_bytes = 0;
+/* The straggler chain: the cooperative kernel is launched IA_STRAGGLER_LEVELS times in a
+ * row.  Level j runs until its queue is empty and then for level_budget << j more iterations per warp; what
+ * still runs then is passed on to level j+1, which packs it ten trajectories to a warp again, in the
+ * lowest-numbered blocks.  The survivors -- the longest trajectories -- so end up in a few dense warps, each
+ * with an SM sub-partition to itself, where the latency of a step is lowest, instead of in thousands of
+ * thinned-out warps that share sub-partitions.  A level lasts twice as long as the one before, so a
+ * trajectory of N steps passes ~log2(N / budget) hand-overs of 256 bytes.  The last level keeps everything. */
+#define IA_BULK_BUDGET 4096u /* the bulk kernel: a warp hands over at the latest this long after the counter ran dry */
+
+/* One run of a generation: what the host entry points have to copy back once its stragglers are done. */
+struct IaPending {
+    ia_outputs host = {nullptr, nullptr, nullptr}; /* host destinations (all NULL for a device-resident run) */
+    ia_outputs dev = {nullptr, nullptr, nullptr};  /* where they sit in the staging */
+    uint64_t n = 0;
+};
+
+/* A generation = the runs whose stragglers ONE launch of the cooperative kernel finishes (ia_set_pipeline).
+ * With depth 0 every run is a generation of its own and everything stays on the caller's stream. */
+struct IaGeneration {
+    IaHand *queue = nullptr;        /* hand-over queue shared by the generation's bulk kernels          */
+    size_t queue_cap = 0;           /* in entries                                                       */
+    IaHand *queue2 = nullptr;       /* second queue of the straggler chain (the levels ping-pong)       */
+    unsigned long long *scratch = nullptr; /* per level j: [2j] entries queued for it, [2j+1] its work counter */
+    cudaStream_t tail = nullptr;    /* stream of the cooperative kernel when depth > 0                  */
+    cudaEvent_t ev_coop[2] = {nullptr, nullptr}; /* around the cooperative kernel                        */
+    cudaEvent_t ev_end = nullptr;   /* after it and after the copies back of the host entry points      */
+    bool used = false;              /* ev_end has been recorded                                         */
+    int n_pending = 0;              /* bulk kernels enqueued, cooperative kernel not yet                */
+    unsigned long long serial = 0;  /* counts the generations this buffer has served                    */
+    IaPending pending[IA_PIPE_MAX];
+    int run_idx[IA_PIPE_MAX] = {};  /* their places in the ring of run events                           */
+    cudaStream_t last_stream = nullptr; /* stream of the generation's latest bulk kernel                */
+    void *stage[IA_PIPE_MAX] = {};  /* device staging of the host entry points, per run of the generation */
+    size_t stage_bytes[IA_PIPE_MAX] = {};
+};
+
+struct IaRunEvents {
+    cudaEvent_t ev[2] = {nullptr, nullptr}; /* around the bulk kernel */
+    int gen = 0;                            /* generation buffer and its serial at the time: where the  */
+    unsigned long long gen_serial = 0;      /* cooperative-kernel time of this run is found             */
 };
 
 struct ia_ctx {
@@ -40,24 +75,23 @@ struct ia_ctx {
     IaParams P;
     double derived[16];
     /* per-launch scratch, a ring so that launches queued behind one another on a stream do not share:
-     * slot = [work counter of the bulk kernel, number handed over, work counter of the cooperative kernel, pad] */
+     * slot = [work counter of the bulk kernel, pad, pad, pad] */
     unsigned long long *counters = nullptr;
     unsigned counter_next = 0;
-    size_t queue_cap = 0; /* entries of one hand-over queue: one per lane of a full bulk grid */
+    size_t queue_cap = 0; /* hand-over entries ONE run can produce: one per lane of a full bulk grid */
     int handoff_lanes = 16;
+    int levels = IA_STRAGGLER_LEVELS;      /* launches of the straggler chain (ia_set_chain) */
+    unsigned level_budget = 8192u;         /* iterations of its first level after the queue ran dry */
     int n_sm = 0;
     IaKernelInfo kinfo[2]; /* 0 bulk, 1 cooperative */
-    /* Run slots.  A run occupies slot seq % max(depth, 1): its hand-over queue, the stream its straggler
-     * kernel runs on (depth > 0; with depth 0 it follows the bulk kernel on the caller's stream), the
-     * events around its kernels and, for the host entry points, its device staging. */
-    int depth = 0;
-    unsigned long long seq = 0;
-    IaSlot slot[IA_PIPE_MAX];
+    int depth = 0;          /* runs per generation - 1 ... 0 = every run on its own (see ia_set_pipeline) */
+    int cur = 0;            /* generation buffer the next run joins */
+    IaGeneration gen[2];    /* two, so that the bulk kernels of one generation overlap the stragglers of the last */
+    unsigned long long seq = 0; /* runs launched so far */
+    IaRunEvents run[IA_RUN_RING];
     cudaStream_t host_stream = nullptr; /* ia_submit_host / ia_run_host */
     std::string err;
 };
-
-#define IA_COUNTER_RING 256 /* slots of 4 x u64 */
 
 static int fail_cuda(ia_ctx *c, const char *what, cudaError_t e) {
     if (c) c->err = std::string(what) + ": " + cudaGetErrorString(e);
@@ -68,16 +102,25 @@ static int fail_inval(ia_ctx *c, const char *what) {
     return IA_EINVAL;
 }
 
-/* allocates what slot k owns (idempotent) */
-static cudaError_t slot_init(ia_ctx *c, int k) {
-    IaSlot &s = c->slot[k];
+/* (re)allocates what generation buffer g owns for `runs` runs per generation */
+static cudaError_t gen_init(ia_ctx *c, int g, int runs) {
+    IaGeneration &G = c->gen[g];
     cudaError_t e = cudaSuccess;
-    if (!s.queue) e = cudaMalloc(&s.queue, c->queue_cap * sizeof(IaHand));
-    /* default priority, like the caller's stream: the next run's bulk kernel (already queued behind this run's
-     * on the caller's stream) takes the SMs first and the straggler kernel fills in as its blocks drain */
-    if (e == cudaSuccess && !s.tail) e = cudaStreamCreateWithFlags(&s.tail, cudaStreamNonBlocking);
-    for (int j = 0; j < 4 && e == cudaSuccess; ++j)
-        if (!s.ev[j]) e = cudaEventCreate(&s.ev[j]);
+    const size_t cap = c->queue_cap * (size_t)runs;
+    if (cap > G.queue_cap) {
+        if (G.queue) cudaFree(G.queue);
+        G.queue = nullptr;
+        G.queue_cap = 0;
+        e = cudaMalloc(&G.queue, cap * sizeof(IaHand));
+        if (e == cudaSuccess) G.queue_cap = cap;
+    }
+    if (e == cudaSuccess && !G.queue2)
+        e = cudaMalloc(&G.queue2, (size_t)c->n_sm * c->kinfo[1].blocks_per_sm * 10 * sizeof(IaHand));
+    if (e == cudaSuccess && !G.scratch) e = cudaMalloc(&G.scratch, IA_SCRATCH_WORDS * sizeof(unsigned long long));
+    if (e == cudaSuccess && !G.tail) e = cudaStreamCreateWithFlags(&G.tail, cudaStreamNonBlocking);
+    for (int j = 0; j < 2 && e == cudaSuccess; ++j)
+        if (!G.ev_coop[j]) e = cudaEventCreate(&G.ev_coop[j]);
+    if (e == cudaSuccess && !G.ev_end) e = cudaEventCreate(&G.ev_end);
     return e;
 }
 
@@ -175,8 +218,10 @@ int ia_create(ia_ctx **out, const ia_species *sp, const ia_trap *tr, double De_K
                                &c->kinfo[k].regs, &c->kinfo[k].local_bytes);
     if (e == cudaSuccess) {
         c->queue_cap = (size_t)c->n_sm * c->kinfo[0].blocks_per_sm * c->kinfo[0].threads_per_block;
-        e = slot_init(c, 0);
+        e = gen_init(c, 0, 1);
     }
+    for (int k = 0; k < IA_RUN_RING && e == cudaSuccess; ++k)
+        for (int j = 0; j < 2 && e == cudaSuccess; ++j) e = cudaEventCreate(&c->run[k].ev[j]);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->host_stream, cudaStreamNonBlocking);
     if (e != cudaSuccess) {
         const int rc = e == cudaErrorMemoryAllocation ? IA_ENOMEM : IA_ECUDA;
@@ -190,18 +235,25 @@ int ia_create(ia_ctx **out, const ia_species *sp, const ia_trap *tr, double De_K
 int ia_destroy(ia_ctx *ctx) {
     if (!ctx) return IA_EINVAL;
     cudaSetDevice(ctx->device);
-    /* runs still in flight finish first: their kernels use the ctx's scratch */
+    /* runs still in flight finish first: their kernels use the ctx's scratch.  (Bulk kernels whose generation
+     * was never joined are on the caller's stream: the caller synchronises that one.) */
     if (ctx->host_stream) cudaStreamSynchronize(ctx->host_stream);
-    for (int k = 0; k < IA_PIPE_MAX; ++k) {
-        IaSlot &s = ctx->slot[k];
-        if (s.used) cudaEventSynchronize(s.ev[2]);
-        if (s.host_used) cudaEventSynchronize(s.ev[3]);
-        if (s.tail) cudaStreamDestroy(s.tail);
-        if (s.queue) cudaFree(s.queue);
-        if (s.stage) cudaFree(s.stage);
-        for (int j = 0; j < 4; ++j)
-            if (s.ev[j]) cudaEventDestroy(s.ev[j]);
+    for (int g = 0; g < 2; ++g) {
+        IaGeneration &G = ctx->gen[g];
+        if (G.used) cudaEventSynchronize(G.ev_end);
+        if (G.tail) cudaStreamDestroy(G.tail);
+        if (G.queue) cudaFree(G.queue);
+        if (G.queue2) cudaFree(G.queue2);
+        if (G.scratch) cudaFree(G.scratch);
+        for (int k = 0; k < IA_PIPE_MAX; ++k)
+            if (G.stage[k]) cudaFree(G.stage[k]);
+        for (int j = 0; j < 2; ++j)
+            if (G.ev_coop[j]) cudaEventDestroy(G.ev_coop[j]);
+        if (G.ev_end) cudaEventDestroy(G.ev_end);
     }
+    for (int k = 0; k < IA_RUN_RING; ++k)
+        for (int j = 0; j < 2; ++j)
+            if (ctx->run[k].ev[j]) cudaEventDestroy(ctx->run[k].ev[j]);
     if (ctx->host_stream) cudaStreamDestroy(ctx->host_stream);
     if (ctx->counters) cudaFree(ctx->counters);
     delete ctx;
@@ -231,43 +283,39 @@ int ia_set_handoff(ia_ctx *ctx, int lanes) {
     return IA_OK;
 }
 
-int ia_set_pipeline(ia_ctx *ctx, int depth) {
+int ia_set_chain(ia_ctx *ctx, int levels, uint32_t budget) {
     if (!ctx) return IA_EINVAL;
-    if (depth < 0 || depth > IA_PIPE_MAX) return fail_inval(ctx, "ia_set_pipeline: depth must be in [0, 16]");
-    cudaError_t e = cudaSetDevice(ctx->device);
-    /* runs in flight keep their slots: let them finish before the slot numbering changes */
-    for (int k = 0; k < IA_PIPE_MAX && e == cudaSuccess; ++k)
-        if (ctx->slot[k].used) e = cudaEventSynchronize(ctx->slot[k].ev[2]);
-    for (int k = 0; k < depth && e == cudaSuccess; ++k) e = slot_init(ctx, k);
-    if (e == cudaErrorMemoryAllocation) {
-        ctx->err = "ia_set_pipeline: hand-over queue allocation failed";
-        return IA_ENOMEM;
-    }
-    if (e != cudaSuccess) return fail_cuda(ctx, "ia_set_pipeline", e);
-    ctx->depth = depth;
-    return IA_OK;
-}
-
-int ia_join(ia_ctx *ctx, void *cuda_stream) {
-    if (!ctx) return IA_EINVAL;
-    cudaError_t e = cudaSetDevice(ctx->device);
-    for (int k = 0; k < IA_PIPE_MAX && e == cudaSuccess; ++k)
-        if (ctx->slot[k].used) e = cudaStreamWaitEvent((cudaStream_t)cuda_stream, ctx->slot[k].ev[2], 0);
-    if (e != cudaSuccess) return fail_cuda(ctx, "ia_join", e);
+    if (levels < 1 || levels > IA_STRAGGLER_LEVELS || budget < 64u)
+        return fail_inval(ctx, "ia_set_chain: need 1 <= levels <= IA_STRAGGLER_LEVELS and budget >= 64");
+    ctx->levels = levels;
+    ctx->level_budget = budget;
     return IA_OK;
 }
 
 int ia_get_timing(ia_ctx *ctx, int runs_back, double *bulk_ms, double *coop_ms) {
     if (!ctx || !bulk_ms || !coop_ms) return IA_EINVAL;
-    const int ring = ctx->depth > 0 ? ctx->depth : 1;
-    if (runs_back < 0 || runs_back >= ring || (unsigned long long)runs_back >= ctx->seq)
+    if (runs_back < 0 || runs_back >= IA_RUN_RING || (unsigned long long)runs_back >= ctx->seq)
         return fail_inval(ctx, "ia_get_timing: that run is no longer (or not yet) on record");
-    IaSlot &s = ctx->slot[(ctx->seq - 1 - (unsigned long long)runs_back) % (unsigned long long)ring];
+    const IaRunEvents &R = ctx->run[(ctx->seq - 1 - (unsigned long long)runs_back) % IA_RUN_RING];
+    if (R.gen < 0) { /* one kernel to the end (IA_PATH_BULK_ONLY / IA_PATH_COOP_ONLY / hand-over off) */
+        cudaError_t e0 = cudaSetDevice(ctx->device);
+        if (e0 == cudaSuccess) e0 = cudaEventSynchronize(R.ev[1]);
+        float a0 = 0.f;
+        if (e0 == cudaSuccess) e0 = cudaEventElapsedTime(&a0, R.ev[0], R.ev[1]);
+        if (e0 != cudaSuccess) return fail_cuda(ctx, "ia_get_timing", e0);
+        *bulk_ms = a0;
+        *coop_ms = 0.0;
+        return IA_OK;
+    }
+    const IaGeneration &G = ctx->gen[R.gen];
+    if (G.serial != R.gen_serial + 1 || !G.used)
+        return fail_inval(ctx, G.serial == R.gen_serial ? "ia_get_timing: the run's stragglers are not enqueued yet (ia_join)"
+                                                        : "ia_get_timing: that run is no longer on record");
     cudaError_t e = cudaSetDevice(ctx->device);
-    if (e == cudaSuccess) e = cudaEventSynchronize(s.ev[2]);
+    if (e == cudaSuccess) e = cudaEventSynchronize(G.ev_end);
     float a = 0.f, b = 0.f;
-    if (e == cudaSuccess) e = cudaEventElapsedTime(&a, s.ev[0], s.ev[1]);
-    if (e == cudaSuccess) e = cudaEventElapsedTime(&b, s.ev[1], s.ev[2]);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&a, R.ev[0], R.ev[1]);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&b, G.ev_coop[0], G.ev_coop[1]);
     if (e != cudaSuccess) return fail_cuda(ctx, "ia_get_timing", e);
     *bulk_ms = a;
     *coop_ms = b;
@@ -344,26 +392,82 @@ static int grid_for(const ia_ctx *ctx, int k, unsigned long long n) {
     return (int)(need < full ? need : full);
 }
 
-/* ia_run proper; *slot_out receives the run slot (only when something was launched, else -1) */
-static int run_impl(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *outputs, cudaStream_t st, int *slot_out) {
-    *slot_out = -1;
+/* Enqueues the cooperative kernel that finishes the hand-overs of generation buffer g, and the copies back
+ * of its host runs.  `st` is the stream the call came in on; with depth 0 everything stays on it. */
+static int flush_generation(ia_ctx *ctx, int g, cudaStream_t st) {
+    IaGeneration &G = ctx->gen[g];
+    if (G.n_pending == 0) return IA_OK;
+    cudaError_t e = cudaSuccess;
+    cudaStream_t ts = st;
+    if (ctx->depth > 0) {
+        /* on the generation's own stream, behind the bulk kernels of all its runs: the caller's stream is free
+         * for the next generation's bulk kernels while this one's longest trajectories finish */
+        ts = G.tail;
+        for (int k = 0; k < G.n_pending && e == cudaSuccess; ++k)
+            e = cudaStreamWaitEvent(ts, ctx->run[G.run_idx[k]].ev[1], 0);
+        if (e != cudaSuccess) return fail_cuda(ctx, "cudaStreamWaitEvent(generation)", e);
+    }
+    IaGen G0;
+    std::memset(&G0, 0, sizeof(G0));
+    IaOut O0 = {nullptr, nullptr, nullptr}; /* every queue entry carries the outputs of its own run */
+    unsigned long long most = (unsigned long long)G.n_pending * ctx->queue_cap / 32ull *
+                              (unsigned long long)(ctx->handoff_lanes > 0 ? ctx->handoff_lanes : 32);
+    IaHand *q_in = G.queue, *q_out = G.queue2;
+    e = cudaEventRecord(G.ev_coop[0], ts);
+    for (int j = 0; j < ctx->levels && e == cudaSuccess; ++j) {
+        IaSched S5;
+        std::memset(&S5, 0, sizeof(S5));
+        S5.q_in = q_in;
+        S5.n_in = G.scratch + 2 * j;
+        S5.counter = G.scratch + 2 * j + 1;
+        if (j + 1 < ctx->levels) {
+            S5.q_out = q_out;
+            S5.n_out = G.scratch + 2 * (j + 1);
+            S5.handoff_lanes = 0;
+            const unsigned long long b = (unsigned long long)ctx->level_budget << j;
+            S5.budget = b > 0xffffffffull ? 0xffffffffu : (unsigned)b;
+        }
+        const int blocks = grid_for(ctx, 1, most);
+        e = ia_launch_persistent(3, ctx->P, G0, O0, S5, blocks, ts);
+        most = (unsigned long long)blocks * 10ull; /* what level j can pass on at most: all it holds */
+        IaHand *t = q_in;
+        q_in = q_out;
+        q_out = t;
+    }
+    if (e == cudaSuccess) e = cudaEventRecord(G.ev_coop[1], ts);
+    for (int k = 0; k < G.n_pending && e == cudaSuccess; ++k) {
+        const IaPending &Q = G.pending[k];
+        if (Q.host.records)
+            e = cudaMemcpyAsync(Q.host.records, Q.dev.records, Q.n * sizeof(ia_record), cudaMemcpyDeviceToHost, ts);
+        if (e == cudaSuccess && Q.host.ic_dump)
+            e = cudaMemcpyAsync(Q.host.ic_dump, Q.dev.ic_dump, Q.n * 14 * sizeof(double), cudaMemcpyDeviceToHost, ts);
+        if (e == cudaSuccess && Q.host.summary)
+            e = cudaMemcpyAsync(Q.host.summary, Q.dev.summary, sizeof(ia_summary), cudaMemcpyDeviceToHost, ts);
+    }
+    if (e == cudaSuccess) e = cudaEventRecord(G.ev_end, ts);
+    if (e != cudaSuccess) return fail_cuda(ctx, "cooperative kernel launch", e);
+    G.used = true;
+    G.serial++;
+    G.n_pending = 0;
+    if (ctx->depth > 0) ctx->cur ^= 1;
+    return IA_OK;
+}
+
+/* ia_run proper.  `pend` (may be NULL) describes the copies back a host entry point wants once the run's
+ * last kernel is done; *deferred says whether they were left to the generation's flush. */
+static int run_impl(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *outputs, cudaStream_t st,
+                    const IaPending *pend, bool *deferred) {
+    if (deferred) *deferred = false;
     ctx->err.clear();
     if (!outputs) return fail_inval(ctx, "outputs is NULL");
-    IaGen G;
+    IaGen Gn;
     unsigned long long warn;
-    int rc = make_gen(ctx, launch, &G, &warn);
+    int rc = make_gen(ctx, launch, &Gn, &warn);
     if (rc != IA_OK) return rc;
-    if (G.n == 0) return IA_OK;
+    if (Gn.n == 0) return IA_OK;
     cudaError_t e = cudaSetDevice(ctx->device);
     if (e != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", e);
-    const int k = ctx->depth > 0 ? (int)(ctx->seq % (unsigned long long)ctx->depth) : 0;
-    IaSlot &sl = ctx->slot[k];
-    /* the slot's queue and events are free again once the run that used them last has ended; with
-     * depth > 0 that run's straggler kernel is on another stream, so the caller's stream waits for it */
-    if (ctx->depth > 0 && sl.used) {
-        e = cudaStreamWaitEvent(st, sl.ev[2], 0);
-        if (e != cudaSuccess) return fail_cuda(ctx, "cudaStreamWaitEvent(slot)", e);
-    }
+    const std::string warn_text = ctx->err;
     unsigned long long *scratch = ctx->counters + 4 * (size_t)(ctx->counter_next++ % IA_COUNTER_RING);
     e = cudaMemsetAsync(scratch, 0, 4 * sizeof(unsigned long long), st);
     if (e != cudaSuccess) return fail_cuda(ctx, "cudaMemsetAsync(counter)", e);
@@ -377,44 +481,53 @@ static int run_impl(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *outp
     std::memset(&S, 0, sizeof(S));
     S.counter = scratch;
     S.warn = warn;
-    cudaStream_t end_stream = st;
-    e = cudaEventRecord(sl.ev[0], st);
-    if (e != cudaSuccess) return fail_cuda(ctx, "cudaEventRecord", e);
-    if (coop_only) {
-        e = ia_launch_persistent(3, ctx->P, G, O, S, grid_for(ctx, 1, G.n), st);
-        if (e == cudaSuccess) e = cudaEventRecord(sl.ev[1], st);
-    } else {
-        if (handoff) {
-            S.q_out = sl.queue;
-            S.n_out = scratch + 1;
-            S.handoff_lanes = ctx->handoff_lanes;
-        }
-        const int blocks = grid_for(ctx, 0, G.n);
-        e = ia_launch_persistent(1, ctx->P, G, O, S, blocks, st);
-        if (e == cudaSuccess) e = cudaEventRecord(sl.ev[1], st);
-        if (e == cudaSuccess && handoff) {
-            /* the straggler kernel resumes what the bulk kernel queued, with a grid that can hold every lane
-             * the bulk grid could have handed over.  depth 0: behind the bulk kernel on the caller's stream.
-             * depth > 0: on the slot's own stream, so that the caller's stream is free for the next run's bulk
-             * kernel while this run's longest trajectories finish. */
-            IaSched S5;
-            std::memset(&S5, 0, sizeof(S5));
-            S5.counter = scratch + 2;
-            S5.q_in = sl.queue;
-            S5.n_in = scratch + 1;
-            if (ctx->depth > 0) {
-                end_stream = sl.tail;
-                e = cudaStreamWaitEvent(end_stream, sl.ev[1], 0);
-            }
-            const unsigned long long most = (unsigned long long)blocks * (unsigned long long)ctx->handoff_lanes;
-            if (e == cudaSuccess) e = ia_launch_persistent(3, ctx->P, G, O, S5, grid_for(ctx, 1, most), end_stream);
-        }
+    const int ridx = (int)(ctx->seq % IA_RUN_RING);
+    IaRunEvents &R = ctx->run[ridx];
+    if (!handoff) {
+        /* one kernel to the end, on the caller's stream: no generation involved */
+        e = cudaEventRecord(R.ev[0], st);
+        if (e == cudaSuccess)
+            e = coop_only ? ia_launch_persistent(3, ctx->P, Gn, O, S, grid_for(ctx, 1, Gn.n), st)
+                          : ia_launch_persistent(1, ctx->P, Gn, O, S, grid_for(ctx, 0, Gn.n), st);
+        if (e == cudaSuccess) e = cudaEventRecord(R.ev[1], st);
+        if (e != cudaSuccess) return fail_cuda(ctx, "persistent kernel launch", e);
+        R.gen = -1;
+        ctx->seq++;
+        ctx->err = warn_text;
+        return IA_OK;
     }
-    if (e == cudaSuccess) e = cudaEventRecord(sl.ev[2], end_stream);
-    if (e != cudaSuccess) return fail_cuda(ctx, "persistent kernel launch", e);
-    sl.used = true;
+    const int g = ctx->depth > 0 ? ctx->cur : 0;
+    IaGeneration &G = ctx->gen[g];
+    /* the generation buffer is free again once the cooperative kernel that read it last has ended */
+    if (G.used) {
+        e = cudaStreamWaitEvent(st, G.ev_end, 0);
+        if (e != cudaSuccess) return fail_cuda(ctx, "cudaStreamWaitEvent(generation buffer)", e);
+    }
+    if (G.n_pending == 0) {
+        e = cudaMemsetAsync(G.scratch, 0, IA_SCRATCH_WORDS * sizeof(unsigned long long), st);
+        if (e != cudaSuccess) return fail_cuda(ctx, "cudaMemsetAsync(generation)", e);
+    }
+    S.q_out = G.queue;
+    S.n_out = G.scratch;
+    S.handoff_lanes = ctx->handoff_lanes;
+    S.budget = IA_BULK_BUDGET;
+    e = cudaEventRecord(R.ev[0], st);
+    if (e == cudaSuccess) e = ia_launch_persistent(1, ctx->P, Gn, O, S, grid_for(ctx, 0, Gn.n), st);
+    if (e == cudaSuccess) e = cudaEventRecord(R.ev[1], st);
+    if (e != cudaSuccess) return fail_cuda(ctx, "bulk kernel launch", e);
+    R.gen = g;
+    R.gen_serial = G.serial;
+    G.pending[G.n_pending] = pend ? *pend : IaPending();
+    G.run_idx[G.n_pending] = ridx;
+    G.last_stream = st;
+    G.n_pending++;
     ctx->seq++;
-    *slot_out = k;
+    if (deferred) *deferred = true;
+    if (G.n_pending >= (ctx->depth > 0 ? ctx->depth : 1)) {
+        rc = flush_generation(ctx, g, st);
+        if (rc != IA_OK) return rc;
+    }
+    ctx->err = warn_text;
     return IA_OK;
 }
 
@@ -428,37 +541,46 @@ static int submit_host_impl(ia_ctx *ctx, const ia_launch *launch, const ia_outpu
         return fail_inval(ctx, "EXPLICIT launch needs y0 and phase");
     cudaError_t e = cudaSetDevice(ctx->device);
     if (e != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", e);
-    const int k = ctx->depth > 0 ? (int)(ctx->seq % (unsigned long long)ctx->depth) : 0;
-    IaSlot &sl = ctx->slot[k];
     cudaStream_t st = ctx->host_stream;
+    /* the staging belongs to the place the run will take in its generation (runs without a hand-over use the
+     * first place of buffer 0, strictly in stream order) */
+    const bool handoff = launch->path == IA_PATH_AUTO && ctx->handoff_lanes > 0;
+    const int g = (handoff && ctx->depth > 0) ? ctx->cur : 0;
+    IaGeneration &G = ctx->gen[g];
+    const int k = handoff ? G.n_pending : 0;
     /* staging layout: [summary 512][records n*64][ic_dump n*14*8][y0 n*12*8][phase n*8] */
     const size_t off_rec = sizeof(ia_summary);
     const size_t off_ic = off_rec + (host_out->records ? n * sizeof(ia_record) : 0);
     const size_t off_y0 = off_ic + (host_out->ic_dump ? n * 14 * sizeof(double) : 0);
     const size_t off_ph = off_y0 + (launch->mode == IA_IC_EXPLICIT ? n * 12 * sizeof(double) : 0);
     const size_t total = off_ph + (launch->mode == IA_IC_EXPLICIT ? n * sizeof(double) : 0);
-    if (total > sl.stage_bytes) {
-        if (sl.host_used) cudaEventSynchronize(sl.ev[3]); /* the slot's previous run still copies from it */
-        if (sl.stage) cudaFree(sl.stage);
-        sl.stage = nullptr;
-        sl.stage_bytes = 0;
-        e = cudaMalloc(&sl.stage, total);
+    if (total > G.stage_bytes[k]) {
+        /* whatever still reads the old staging finishes first */
+        e = cudaStreamSynchronize(st);
+        if (e == cudaSuccess && G.used) e = cudaEventSynchronize(G.ev_end);
+        if (e != cudaSuccess) return fail_cuda(ctx, "synchronise before staging reallocation", e);
+        if (G.stage[k]) cudaFree(G.stage[k]);
+        G.stage[k] = nullptr;
+        G.stage_bytes[k] = 0;
+        e = cudaMalloc(&G.stage[k], total);
         if (e != cudaSuccess) {
             ctx->err = "device staging allocation failed";
             return IA_ENOMEM;
         }
-        sl.stage_bytes = total;
+        G.stage_bytes[k] = total;
     }
-    if (sl.host_used) { /* the staging is free again once the slot's previous copies back are done */
-        e = cudaStreamWaitEvent(st, sl.ev[3], 0);
+    if (G.used) { /* the copies back of the generation that used this staging last are behind ev_end */
+        e = cudaStreamWaitEvent(st, G.ev_end, 0);
         if (e != cudaSuccess) return fail_cuda(ctx, "cudaStreamWaitEvent(staging)", e);
     }
-    char *base = (char *)sl.stage;
+    char *base = (char *)G.stage[k];
     ia_launch L = *launch;
-    ia_outputs O;
-    O.summary = (ia_summary *)base;
-    O.records = host_out->records ? (ia_record *)(base + off_rec) : nullptr;
-    O.ic_dump = host_out->ic_dump ? (double *)(base + off_ic) : nullptr;
+    IaPending Q;
+    Q.host = *host_out;
+    Q.n = n;
+    Q.dev.summary = (ia_summary *)base;
+    Q.dev.records = host_out->records ? (ia_record *)(base + off_rec) : nullptr;
+    Q.dev.ic_dump = host_out->ic_dump ? (double *)(base + off_ic) : nullptr;
     e = cudaMemsetAsync(base, 0, sizeof(ia_summary), st);
     if (e != cudaSuccess) return fail_cuda(ctx, "cudaMemsetAsync(summary)", e);
     if (launch->mode == IA_IC_EXPLICIT) {
@@ -469,22 +591,18 @@ static int submit_host_impl(ia_ctx *ctx, const ia_launch *launch, const ia_outpu
         L.y0 = (const double *)(base + off_y0);
         L.phase = (const double *)(base + off_ph);
     }
-    int used = -1;
-    int rc = run_impl(ctx, &L, &O, st, &used);
-    if (rc != IA_OK) return rc;
+    bool deferred = false;
+    int rc = run_impl(ctx, &L, &Q.dev, st, &Q, &deferred);
+    if (rc != IA_OK || deferred) return rc;
+    /* no hand-over: the run ended on st, the copies back follow it there */
     const std::string warn_text = ctx->err;
-    /* the copies back follow the run's last kernel: on the slot's straggler stream when there is one */
-    cudaStream_t back = st;
-    if (ctx->depth > 0 && launch->path == IA_PATH_AUTO && ctx->handoff_lanes > 0) back = sl.tail;
-    if (host_out->records)
-        e = cudaMemcpyAsync(host_out->records, O.records, n * sizeof(ia_record), cudaMemcpyDeviceToHost, back);
-    if (e == cudaSuccess && host_out->ic_dump)
-        e = cudaMemcpyAsync(host_out->ic_dump, O.ic_dump, n * 14 * sizeof(double), cudaMemcpyDeviceToHost, back);
-    if (e == cudaSuccess && host_out->summary)
-        e = cudaMemcpyAsync(host_out->summary, O.summary, sizeof(ia_summary), cudaMemcpyDeviceToHost, back);
-    if (e == cudaSuccess) e = cudaEventRecord(sl.ev[3], back);
+    if (Q.host.records)
+        e = cudaMemcpyAsync(Q.host.records, Q.dev.records, n * sizeof(ia_record), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && Q.host.ic_dump)
+        e = cudaMemcpyAsync(Q.host.ic_dump, Q.dev.ic_dump, n * 14 * sizeof(double), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && Q.host.summary)
+        e = cudaMemcpyAsync(Q.host.summary, Q.dev.summary, sizeof(ia_summary), cudaMemcpyDeviceToHost, st);
     if (e != cudaSuccess) return fail_cuda(ctx, "D2H copy", e);
-    sl.host_used = true;
     ctx->err = warn_text;
     return IA_OK;
 }
@@ -493,8 +611,46 @@ extern "C" {
 
 int ia_run(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *outputs, void *cuda_stream) {
     if (!ctx) return IA_EINVAL;
-    int slot;
-    return run_impl(ctx, launch, outputs, (cudaStream_t)cuda_stream, &slot);
+    return run_impl(ctx, launch, outputs, (cudaStream_t)cuda_stream, nullptr, nullptr);
+}
+
+int ia_join(ia_ctx *ctx, void *cuda_stream) {
+    if (!ctx) return IA_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    cudaError_t e = cudaSetDevice(ctx->device);
+    if (e != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", e);
+    for (int g = 0; g < 2; ++g) {
+        const int rc = flush_generation(ctx, g, st);
+        if (rc != IA_OK) return rc;
+    }
+    for (int g = 0; g < 2 && e == cudaSuccess; ++g)
+        if (ctx->gen[g].used) e = cudaStreamWaitEvent(st, ctx->gen[g].ev_end, 0);
+    if (e != cudaSuccess) return fail_cuda(ctx, "ia_join", e);
+    return IA_OK;
+}
+
+int ia_set_pipeline(ia_ctx *ctx, int depth) {
+    if (!ctx) return IA_EINVAL;
+    if (depth < 0 || depth > IA_PIPE_MAX) return fail_inval(ctx, "ia_set_pipeline: depth must be in [0, 64]");
+    cudaError_t e = cudaSetDevice(ctx->device);
+    if (e != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", e);
+    /* runs in flight keep the old layout: enqueue what is pending and let everything finish */
+    for (int g = 0; g < 2; ++g) {
+        const int rc = flush_generation(ctx, g, ctx->gen[g].last_stream);
+        if (rc != IA_OK) return rc;
+    }
+    for (int g = 0; g < 2 && e == cudaSuccess; ++g)
+        if (ctx->gen[g].used) e = cudaEventSynchronize(ctx->gen[g].ev_end);
+    if (e == cudaSuccess) e = gen_init(ctx, 0, depth > 0 ? depth : 1);
+    if (e == cudaSuccess && depth > 0) e = gen_init(ctx, 1, depth);
+    if (e == cudaErrorMemoryAllocation) {
+        ctx->err = "ia_set_pipeline: hand-over queue allocation failed";
+        return IA_ENOMEM;
+    }
+    if (e != cudaSuccess) return fail_cuda(ctx, "ia_set_pipeline", e);
+    ctx->depth = depth;
+    ctx->cur = 0;
+    return IA_OK;
 }
 
 int ia_submit_host(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *host_outputs) {
@@ -504,12 +660,9 @@ int ia_submit_host(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *host_
 
 int ia_wait(ia_ctx *ctx) {
     if (!ctx) return IA_EINVAL;
-    cudaError_t e = cudaSetDevice(ctx->device);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->host_stream);
-    for (int k = 0; k < IA_PIPE_MAX && e == cudaSuccess; ++k) {
-        if (ctx->slot[k].used) e = cudaEventSynchronize(ctx->slot[k].ev[2]);
-        if (e == cudaSuccess && ctx->slot[k].host_used) e = cudaEventSynchronize(ctx->slot[k].ev[3]);
-    }
+    int rc = ia_join(ctx, ctx->host_stream);
+    if (rc != IA_OK) return rc;
+    cudaError_t e = cudaStreamSynchronize(ctx->host_stream);
     if (e != cudaSuccess) return fail_cuda(ctx, "ia_wait", e);
     return IA_OK;
 }

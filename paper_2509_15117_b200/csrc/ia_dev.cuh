@@ -302,8 +302,25 @@ IA_DEV void ia_dp5_attempt(const IaParams &P, const IaLane<LPT> &L, const IaVec<
     /* the stage cosines depend on (tf, h) only: independent chains that fill the latency of the serial
      * r^2 -> 1/r^2 -> force chain; each is released two stages ahead of its use */
     const double hc2 = h * IA_C2, hc3 = h * IA_C3, hc4 = h * IA_C4, hc5 = h * IA_C5;
-    const double cs2 = ia_cos_folded(ia_fma<FUSED>(P.omega, tf + hc2, phase));
-    const double cs3 = ia_cos_folded(ia_fma<FUSED>(P.omega, tf + hc3, phase));
+    double cs2, cs3, cs4 = 0.0, cs5 = 0.0, cs1 = 0.0;
+    if (LPT == 1) {
+        cs2 = ia_cos_folded(ia_fma<FUSED>(P.omega, tf + hc2, phase));
+        cs3 = ia_cos_folded(ia_fma<FUSED>(P.omega, tf + hc3, phase));
+    } else {
+        /* three lanes share the five cosines: lane k of the group evaluates the stage times (t2, t3, t4)[k] and
+         * (t5, t1, t1)[k] -- the same function of the same argument as in the one-lane layout -- and the group
+         * reads them with shuffles: two evaluations per lane and step instead of five */
+        const unsigned k = L.axis0;
+        const double ta = tf + (k == 0u ? hc2 : (k == 1u ? hc3 : hc4));
+        const double tb = tf + (k == 0u ? hc5 : h);
+        const double ca = ia_cos_folded(ia_fma<FUSED>(P.omega, ta, phase));
+        const double cb = ia_cos_folded(ia_fma<FUSED>(P.omega, tb, phase));
+        cs2 = __shfl_sync(IA_FULL, ca, (int)L.gbase);
+        cs3 = __shfl_sync(IA_FULL, ca, (int)L.gbase + 1);
+        cs4 = __shfl_sync(IA_FULL, ca, (int)L.gbase + 2);
+        cs5 = __shfl_sync(IA_FULL, cb, (int)L.gbase);
+        cs1 = __shfl_sync(IA_FULL, cb, (int)L.gbase + 1);
+    }
     double Xi[NA], Xa[NA], D[3], r2, s;
     double A2i[NA], A2a[NA], A3i[NA], A3a[NA], A4i[NA], A4a[NA], A5i[NA], A5a[NA], A6i[NA], A6a[NA];
 #define IA_F(a, b, c) ia_fma<FUSED>(a, b, c)
@@ -314,9 +331,11 @@ IA_DEV void ia_dp5_attempt(const IaParams &P, const IaLane<LPT> &L, const IaVec<
         Xa[a] = IA_F(hc2, Y.va[a], Y.xa[a]);
     }
     ia_accel<LPT, FUSED>(P, L, Xi, Xa, cs2, A2i, A2a, D, r2, s);
-    double t4 = tf + hc4;
-    IA_TIE(t4, A2a[0]);
-    const double cs4 = ia_cos_folded(ia_fma<FUSED>(P.omega, t4, phase));
+    if (LPT == 1) {
+        double t4 = tf + hc4;
+        IA_TIE(t4, A2a[0]);
+        cs4 = ia_cos_folded(ia_fma<FUSED>(P.omega, t4, phase));
+    }
     /* stage 3 */
     {
         const double g1 = hh * IA_AB31;
@@ -327,9 +346,11 @@ IA_DEV void ia_dp5_attempt(const IaParams &P, const IaLane<LPT> &L, const IaVec<
         }
         ia_accel<LPT, FUSED>(P, L, Xi, Xa, cs3, A3i, A3a, D, r2, s);
     }
-    double t5 = tf + hc5;
-    IA_TIE(t5, A3a[0]);
-    const double cs5 = ia_cos_folded(ia_fma<FUSED>(P.omega, t5, phase));
+    if (LPT == 1) {
+        double t5 = tf + hc5;
+        IA_TIE(t5, A3a[0]);
+        cs5 = ia_cos_folded(ia_fma<FUSED>(P.omega, t5, phase));
+    }
     /* stage 4 */
     {
         const double g1 = hh * IA_AB41, g2 = hh * IA_AB42;
@@ -340,9 +361,11 @@ IA_DEV void ia_dp5_attempt(const IaParams &P, const IaLane<LPT> &L, const IaVec<
         }
         ia_accel<LPT, FUSED>(P, L, Xi, Xa, cs4, A4i, A4a, D, r2, s);
     }
-    double t1 = tf + h; /* stages 6 and 7 share the time t + h */
-    IA_TIE(t1, A4a[0]);
-    const double cs1 = ia_cos_folded(ia_fma<FUSED>(P.omega, t1, phase));
+    if (LPT == 1) {
+        double t1 = tf + h; /* stages 6 and 7 share the time t + h */
+        IA_TIE(t1, A4a[0]);
+        cs1 = ia_cos_folded(ia_fma<FUSED>(P.omega, t1, phase));
+    }
     /* stage 5 */
     {
         const double g1 = hh * IA_AB51, g2 = hh * IA_AB52, g3 = hh * IA_AB53;

@@ -21,6 +21,7 @@
 #include "ia_kernels.cuh"
 
 #define IA_THREADS 32
+#define IA_INNER 64u /* step attempts between two looks at the work counter / hand-over rules */
 
 enum { MODE_IDLE = 0, MODE_RUN = 1, MODE_LOC = 2 };
 
@@ -143,7 +144,10 @@ __device__ __forceinline__ void ia_park(const IaLane<LPT> &L, IaVec<LPT> &Y) {
 
 /* ---- K1 / K5 ---------------------------------------------------------------------------------- */
 
-template <int LPT>
+/* RESUME: the kernel takes its trajectories from a hand-over queue (a level of the straggler chain) instead of
+ * generating them; a compile-time switch, so that the chain's kernel carries neither the generator nor its
+ * registers -- the latency of its step loop is what the longest trajectories of a launch wait for. */
+template <int LPT, bool RESUME>
 __global__ void __launch_bounds__(IA_THREADS, LPT == 1 ? 12 : 16)
 ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__ IaGen G, const IaOut O,
                      const IaSched S) {
@@ -154,23 +158,33 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
     IaVec<LPT> Y;
     double tf = 0.0, h = 0.0;
     unsigned n_per = 0, steps_acc = 0;
-    /* rarely touched per-group state lives in shared memory, not in registers */
-    __shared__ double sh_t_first[IA_THREADS], sh_t_last[IA_THREADS], sh_phase[IA_THREADS], sh_s_old[IA_THREADS];
-    __shared__ unsigned long long sh_slot[IA_THREADS];
-    __shared__ unsigned sh_steps_in[IA_THREADS], sh_n_coll[IA_THREADS], sh_n_tp[IA_THREADS], sh_n_loc[IA_THREADS],
-        sh_steps_rej[IA_THREADS];
-    double &t_first = sh_t_first[threadIdx.x], &t_last = sh_t_last[threadIdx.x], &phase = sh_phase[threadIdx.x],
-           &s_old = sh_s_old[threadIdx.x];
+    /* rarely touched per-group state lives in shared memory, not in registers: one struct of arrays, so that
+     * a lane reaches all of it from two address registers (8-byte and 4-byte members) */
+    __shared__ struct {
+        double t_first[IA_THREADS], t_last[IA_THREADS], phase[IA_THREADS], s_old[IA_THREADS];
+        unsigned long long slot[IA_THREADS];
+        ia_record *rec[IA_THREADS];   /* outputs of the run the group's trajectory belongs to */
+        ia_summary *sum[IA_THREADS];
+        unsigned steps_in[IA_THREADS], n_coll[IA_THREADS], n_tp[IA_THREADS], n_loc[IA_THREADS], steps_rej[IA_THREADS],
+            cnt[IA_THREADS];
+    } sh;
+    double &t_first = sh.t_first[threadIdx.x], &t_last = sh.t_last[threadIdx.x], &phase = sh.phase[threadIdx.x],
+           &s_old = sh.s_old[threadIdx.x];
     phase = 0.0; s_old = 0.0;
-    unsigned long long &slot = sh_slot[threadIdx.x];
-    unsigned &steps_in = sh_steps_in[threadIdx.x], &n_coll = sh_n_coll[threadIdx.x], &n_tp = sh_n_tp[threadIdx.x],
-             &n_loc = sh_n_loc[threadIdx.x], &steps_rej = sh_steps_rej[threadIdx.x];
+    unsigned long long &slot = sh.slot[threadIdx.x];
+    ia_record *&out_rec = sh.rec[threadIdx.x];
+    ia_summary *&out_sum = sh.sum[threadIdx.x];
+    out_rec = O.records; out_sum = O.summary;
+    unsigned &steps_in = sh.steps_in[threadIdx.x], &n_coll = sh.n_coll[threadIdx.x], &n_tp = sh.n_tp[threadIdx.x],
+             &n_loc = sh.n_loc[threadIdx.x], &steps_rej = sh.steps_rej[threadIdx.x];
+    unsigned &cnt = sh.cnt[threadIdx.x]; /* warp-uniform: step attempts since the queue ran dry */
+    cnt = 0;
     t_first = 0.0; t_last = 0.0; slot = 0; steps_in = 0; n_coll = 0; n_tp = 0; n_loc = 0; steps_rej = 0;
     int mode = MODE_IDLE;
     bool failed = false;
     bool wexh = false; /* warp-uniform: the work counter is empty */
     ia_park<LPT>(L, Y);
-    if (O.summary != nullptr && threadIdx.x == 0 && S.q_in == nullptr) {
+    if (!RESUME && O.summary != nullptr && threadIdx.x == 0) {
         const unsigned long long t0 = ia_globaltimer();
         if (blockIdx.x == 0) {
             atomicCAS((unsigned long long *)&O.summary->t_start_ns, 0ull, t0);
@@ -178,25 +192,39 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
         }
     }
 
+    constexpr unsigned long long PER_WARP = (LPT == 1) ? 32ull : 10ull; /* trajectories a warp holds */
+    /* A kernel that resumes from a queue deals the first gridDim.x * PER_WARP entries out by block index, so that
+     * when the queue is short the work sits in the lowest-numbered blocks -- which the hardware spreads over the
+     * SMs -- instead of wherever the race for the counter ends; the counter serves the rest of the queue. */
+    constexpr bool resume = RESUME;
+#define IA_DEALT (resume ? (unsigned long long)gridDim.x * PER_WARP : 0ull)
+#define IA_N_TOTAL (resume ? *S.n_in : G.n) /* final: the producer kernel has ended */
+    bool first_refill = resume;
+
     for (;;) {
+        const bool was_exh = wexh;
         /* ---- refill idle groups from the global work counter (a12) ---- */
         const bool want = L.valid && (mode == MODE_IDLE) && !wexh;
         const unsigned wm = __ballot_sync(IA_FULL, want && L.leader);
         if (wm) {
             const int first = __ffs(wm) - 1;
             unsigned long long base = 0;
-            if ((int)lane == first) base = atomicAdd(S.counter, (unsigned long long)__popc(wm));
-            base = __shfl_sync(IA_FULL, base, first);
+            if (first_refill) {
+                base = (unsigned long long)blockIdx.x * PER_WARP;
+                first_refill = false;
+            } else {
+                if ((int)lane == first) base = IA_DEALT + atomicAdd(S.counter, (unsigned long long)__popc(wm));
+                base = __shfl_sync(IA_FULL, base, first);
+            }
             const unsigned long long j = base + __popc(wm & ((1u << L.gbase) - 1u));
-            const unsigned long long n_total = (S.q_in != nullptr) ? *S.n_in : G.n;
-            const bool got = want && (j < n_total);
+            const bool got = want && (j < IA_N_TOTAL);
             if (__any_sync(IA_FULL, want && !got)) {
-                if (!wexh && O.summary != nullptr && S.q_in == nullptr && lane == 0)
+                if (!wexh && O.summary != nullptr && !resume && lane == 0)
                     atomicCAS((unsigned long long *)&O.summary->t_first_idle_ns, 0ull, ia_globaltimer());
                 wexh = true;
             }
             if (got) {
-                if (S.q_in != nullptr) {
+                if (resume) {
                     /* resume a trajectory the bulk kernel handed over */
                     const IaHand *H = S.q_in + j;
 #pragma unroll
@@ -208,9 +236,10 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
                     }
                     tf = H->tf; h = H->h; phase = H->phase; s_old = H->s_old;
                     t_first = H->t_first; t_last = H->t_last; slot = H->slot;
+                    out_rec = H->records; out_sum = H->summary;
                     n_per = H->n_per; n_coll = H->n_coll; n_tp = H->n_tp;
                     steps_acc = H->steps_acc; steps_rej = H->steps_rej; failed = H->failed != 0u;
-                    steps_in = steps_acc + steps_rej;
+                    steps_in = H->steps_in;
                     n_loc = 0;
                     mode = MODE_RUN;
                 } else {
@@ -227,6 +256,7 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
                         o[13] = ic.E_au;
                     }
                     slot = j;
+                    out_rec = O.records; out_sum = O.summary;
                     tf = 0.0; n_per = 0; n_coll = 0; n_tp = 0; steps_acc = 0; steps_rej = 0; n_loc = 0; steps_in = 0;
                     t_first = 0.0; t_last = 0.0; failed = false;
                     phase = ic.phase;
@@ -291,27 +321,45 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
             }
         }
 
-        /* ---- hand the last running lanes of a drained warp over to the straggler kernel ---- */
-        if (LPT == 1 && S.q_out != nullptr && wexh) {
-            const unsigned am = __ballot_sync(IA_FULL, mode == MODE_RUN);
+        /* a warp whose groups are all busy never asks the counter: let it notice an empty queue anyway */
+        if (!wexh) {
+            unsigned long long c = 0;
+            if (lane == 0) c = IA_DEALT + *(volatile unsigned long long *)S.counter;
+            c = __shfl_sync(IA_FULL, c, 0);
+            if (c >= IA_N_TOTAL) wexh = true;
+        }
+        if (wexh && !was_exh) cnt = 0u;
+
+        /* ---- hand what still runs in a drained warp over to the next kernel of the chain: when few
+         * trajectories are left in the warp (handoff_lanes), or when the warp has gone on for `budget`
+         * iterations since the queue ran dry (so that no warp holds a level of the chain up) ---- */
+        if (S.q_out != nullptr && wexh) {
+            const unsigned am = __ballot_sync(IA_FULL, mode == MODE_RUN && L.leader); /* one bit per trajectory */
             const unsigned lm = __ballot_sync(IA_FULL, mode == MODE_LOC);
-            if (am != 0u && lm == 0u && __popc(am) <= S.handoff_lanes) {
+            if (am != 0u && lm == 0u && (__popc(am) <= S.handoff_lanes || cnt >= S.budget)) {
                 const int first = __ffs(am) - 1;
                 unsigned long long base = 0;
                 if ((int)lane == first) base = atomicAdd(S.n_out, (unsigned long long)__popc(am));
                 base = __shfl_sync(IA_FULL, base, first);
-                if (mode == MODE_RUN) {
-                    IaHand *H = S.q_out + base + __popc(am & ((1u << lane) - 1u));
+                if (mode == MODE_RUN && L.valid) {
+                    /* every lane of the group writes the axes it holds, the leader the rest */
+                    IaHand *H = S.q_out + base + __popc(am & ((1u << L.gbase) - 1u));
 #pragma unroll
                     for (int a = 0; a < NA; ++a) {
-                        H->x[a] = Y.xi[a];  H->x[3 + a] = Y.xa[a];
-                        H->v[a] = Y.vi[a];  H->v[3 + a] = Y.va[a];
-                        H->A1[a] = Y.Ai[a]; H->A1[3 + a] = Y.Aa[a];
+                        const unsigned ax = L.axis0 + a;
+                        H->x[ax] = Y.xi[a];  H->x[3 + ax] = Y.xa[a];
+                        H->v[ax] = Y.vi[a];  H->v[3 + ax] = Y.va[a];
+                        H->A1[ax] = Y.Ai[a]; H->A1[3 + ax] = Y.Aa[a];
                     }
-                    H->tf = tf; H->h = h; H->phase = phase; H->s_old = s_old;
-                    H->t_first = t_first; H->t_last = t_last; H->slot = slot;
-                    H->n_per = n_per; H->n_coll = n_coll; H->n_tp = n_tp;
-                    H->steps_acc = steps_acc; H->steps_rej = steps_rej; H->failed = failed ? 1u : 0u;
+                    if (L.leader) {
+                        H->tf = tf; H->h = h; H->phase = phase; H->s_old = s_old;
+                        H->t_first = t_first; H->t_last = t_last; H->slot = slot;
+                        H->records = out_rec; H->summary = out_sum;
+                        H->n_per = n_per; H->n_coll = n_coll; H->n_tp = n_tp;
+                        H->steps_acc = steps_acc; H->steps_rej = steps_rej; H->failed = failed ? 1u : 0u;
+                        /* steps taken before the first hand-over (the bulk kernel's share of the trajectory) */
+                        H->steps_in = (resume) ? steps_in : steps_acc + steps_rej;
+                    }
                     mode = MODE_IDLE;
                 }
             }
@@ -321,13 +369,21 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
             continue;
         }
 
-        /* ---- one DP5(4) attempt for every lane (idle lanes step a harmless dummy state) ---- */
+        /* ---- the step loop proper: up to IA_INNER attempts without looking at the counter, the queues or the
+         * budget; it is left as soon as a trajectory of the warp terminates.  Everything that is only needed
+         * between two visits here stays out of its registers. ---- */
+        int fin;          /* >= 0: terminate with this status */
+        double t_fin;
+        bool fin_exit;
+        IaVec<LPT> N;
+        unsigned it = 0;
+        do {
+        /* one DP5(4) attempt for every lane (idle lanes step a harmless dummy state) */
         const bool run = (mode == MODE_RUN), loc = (mode == MODE_LOC);
         /* clip the last step to land on t_max (R5/R8) */
         const double rem = (P.t_max_rf - (double)n_per) * P.T_rf - tf;
         const bool last = run && (h >= rem);
         h = last ? rem : h;
-        IaVec<LPT> N;
         IaStepOut so;
         ia_dp5_attempt<LPT, true>(P, L, Y, tf, phase, h, N, so);
 
@@ -365,7 +421,7 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
             ++n_loc;
             loc_done = g_small || n_loc >= 8u;
         }
-        const bool fin_exit = (exitc && g_small) || loc_done;
+        fin_exit = (exitc && g_small) || loc_done;
         const bool newton = (exitc && !g_small) || (loc && !loc_done);
         const bool commit = acc && !exitc;
         const bool underflow = rej && (hs <= P.h_min);
@@ -398,8 +454,8 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
             if (exitc) n_loc = 0u;
             mode = MODE_LOC;
         }
-        int fin = -1; /* >= 0: terminate with this status */
-        double t_fin = now + hs;
+        fin = -1;
+        t_fin = now + hs;
         if (fin_exit) {
             fin = 0;
         } else if (commit && last) {
@@ -412,6 +468,9 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
             fin = 4;
             t_fin = (double)n_per * P.T_rf + tf;
         }
+        ++it;
+        } while (!__any_sync(IA_FULL, fin >= 0) && it < IA_INNER);
+        cnt += it;
 
         if (__any_sync(IA_FULL, fin >= 0)) {
             /* observables (R10) + record (a10) + ensemble reduction (a11); the velocity vectors of the
@@ -427,7 +486,7 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
             if (fin >= 0) {
                 if (L.leader) {
                     const double ke = (0.5 * P.m_i) * ia_dot3<true>(VI, VI);
-                    if (O.records != nullptr) {
+                    if (out_rec != nullptr) {
                         ia_record r;
                         r.ke_ion = ke;
                         r.t_dwell = t_fin;
@@ -439,17 +498,18 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
                         r.steps_rej = (uint16_t)min(steps_rej, 65535u);
                         r.status = (uint8_t)fin;
                         r.n_loc = (uint8_t)n_loc;
-                        O.records[slot] = r;
+                        out_rec[slot] = r;
                     }
-                    if (O.summary != nullptr) {
-                        ia_summary *Sm = O.summary;
+                    if (out_sum != nullptr) {
+                        ia_summary *Sm = out_sum;
                         atomicAdd((unsigned long long *)&Sm->n_done, 1ull);
                         atomicAdd((unsigned long long *)&Sm->n_status[fin], 1ull);
                         if (n_coll >= 2u) atomicAdd((unsigned long long *)&Sm->n_complex, 1ull);
                         atomicAdd((unsigned long long *)&Sm->steps_acc, (unsigned long long)steps_acc);
                         atomicAdd((unsigned long long *)&Sm->steps_rej, (unsigned long long)steps_rej);
                         atomicAdd((unsigned long long *)&Sm->steps_loc, (unsigned long long)n_loc);
-                        if (S.q_in != nullptr) {
+                        if (resume) {
+                            atomicMax((unsigned long long *)&Sm->t_end_ns, ia_globaltimer());
                             atomicAdd((unsigned long long *)&Sm->n_handoff, 1ull);
                             atomicAdd((unsigned long long *)&Sm->steps_coop,
                                       (unsigned long long)(steps_acc + steps_rej - steps_in + n_loc));
@@ -469,7 +529,7 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
     if (O.summary != nullptr && lane == 0) {
         const unsigned long long t1 = ia_globaltimer();
         atomicMax((unsigned long long *)&O.summary->t_end_ns, t1);
-        if (S.q_in == nullptr) atomicMax((unsigned long long *)&O.summary->t_bulk_end_ns, t1);
+        if (!resume) atomicMax((unsigned long long *)&O.summary->t_bulk_end_ns, t1);
     }
 }
 
@@ -560,16 +620,21 @@ __global__ void ia_trace_kernel(const __grid_constant__ IaParams P, IaY12 y0, do
 
 cudaError_t ia_launch_persistent(int lanes_per_traj, const IaParams &P, const IaGen &G, const IaOut &O,
                                  const IaSched &S, int grid_blocks, cudaStream_t st) {
-    if (lanes_per_traj == 1)
-        ia_persistent_kernel<1><<<grid_blocks, IA_THREADS, 0, st>>>(P, G, O, S);
-    else
-        ia_persistent_kernel<3><<<grid_blocks, IA_THREADS, 0, st>>>(P, G, O, S);
+    if (lanes_per_traj == 1) {
+        if (S.q_in != nullptr) return cudaErrorInvalidValue; /* only the cooperative kernel resumes from a queue */
+        ia_persistent_kernel<1, false><<<grid_blocks, IA_THREADS, 0, st>>>(P, G, O, S);
+    } else if (S.q_in != nullptr) {
+        ia_persistent_kernel<3, true><<<grid_blocks, IA_THREADS, 0, st>>>(P, G, O, S);
+    } else {
+        ia_persistent_kernel<3, false><<<grid_blocks, IA_THREADS, 0, st>>>(P, G, O, S);
+    }
     return cudaGetLastError();
 }
 
 cudaError_t ia_persistent_info(int lanes_per_traj, int *blocks_per_sm, int *threads_per_block, int *regs,
                                int *local_bytes) {
-    const void *fn = lanes_per_traj == 1 ? (const void *)ia_persistent_kernel<1> : (const void *)ia_persistent_kernel<3>;
+    const void *fn = lanes_per_traj == 1 ? (const void *)ia_persistent_kernel<1, false>
+                                         : (const void *)ia_persistent_kernel<3, true>;
     cudaFuncAttributes fa;
     cudaError_t e = cudaFuncGetAttributes(&fa, fn);
     if (e != cudaSuccess) return e;

@@ -33,7 +33,11 @@ struct IaHand {
     double tf, h, phase, s_old, t_first, t_last;
     unsigned long long slot;
     unsigned n_per, n_coll, n_tp, steps_acc, steps_rej, failed;
-    unsigned long long pad[4];
+    ia_record *records;  /* where its outcome goes: the outputs of the run it came from, so that one straggler */
+    ia_summary *summary; /* kernel can finish the hand-overs of several runs (ia_set_pipeline)                */
+    unsigned steps_in;   /* attempted steps before the first hand-over */
+    unsigned pad32;
+    unsigned long long pad;
 };
 static_assert(sizeof(IaHand) == 256, "IaHand is 256 bytes");
 
@@ -44,7 +48,8 @@ struct IaSched {
     const unsigned long long *n_in;  /* ... their number (device memory, written by the producing kernel) */
     IaHand *q_out;                   /* non-NULL: hand unfinished trajectories over to this queue ...     */
     unsigned long long *n_out;       /* ... counting them here                                           */
-    int handoff_lanes;               /* ... once the counter is empty and <= this many lanes of a warp run */
+    int handoff_lanes;               /* ... once the counter is empty and <= this many trajectories of a warp run */
+    unsigned budget;                 /* ... or once it has run this many iterations since the counter ran dry */
     unsigned long long warn;
 };
 
