@@ -30,7 +30,7 @@ ATOMS: Dict[str, Dict[str, float]] = {
     "Cs133": {"m_u": 132.905, "alpha": 401.0},
 }
 
-MODE_EXPLICIT, MODE_GRID, MODE_PHILOX = 0, 1, 2
+MODE_EXPLICIT, MODE_GRID, MODE_PHILOX, MODE_THERMAL = 0, 1, 2, 3
 
 
 @dataclass(frozen=True)
@@ -71,6 +71,8 @@ class Launch:
     cell: int = 0
     first_index: int = 0
     path: int = 0              # 0 production kernel pair, 1 bulk kernel only, 2 cooperative kernel only
+    T_atom_uK: float = 0.0     # THERMAL: bath temperature
+    T_ion_uK: float = 0.0      # THERMAL: ion temperature (the paper's thermal runs use 10 uK)
 
 
 @dataclass(frozen=True)
@@ -142,6 +144,24 @@ def config4(n_total: int = 300_000_000, batch: int = 2 ** 24, seed: int = DEFAUL
                                  E_max_uK=100.0, seed=seed, cell=200, first_index=first)))
         first += n
     return cells
+
+
+THERMAL_T_UK = [1.0, 3.0, 10.0, 30.0, 100.0]
+
+
+def thermal(atom: str = "Rb87", T_atom_uK: float = 1.0, De_K: float = 1.0, n: int = 2 ** 20,
+            seed: int = DEFAULT_SEED) -> Cell:
+    """One bar of the paper's Fig. 3: thermal run of Yb+ with
+    `atom` at bath temperature T, ion at 10 uK, atom uniform on the r0 sphere with Maxwell-Boltzmann velocity
+    (v_r < 0 enforced), uniform rf phase.  Philox cell = 300 + 25*[De = 100 K] + 5*species + temperature index
+    (or 399 for a temperature off the list)."""
+    si = SPECIES_ORDER.index(atom)
+    ti = THERMAL_T_UK.index(T_atom_uK) if T_atom_uK in THERMAL_T_UK else None
+    cell = 399 if ti is None else 300 + (25 if De_K >= 50.0 else 0) + 5 * si + ti
+    p = replace(Params().with_atom(atom), De_K=De_K)
+    return Cell(f"thermal_{atom}_{T_atom_uK:g}uK_De{De_K:g}K", p,
+                Launch(mode=MODE_THERMAL, n=n, domain=1, phase_mode=1, seed=seed, cell=cell,
+                       T_atom_uK=T_atom_uK, T_ion_uK=10.0))
 
 
 def subgrid_indices(n_side: int, every: int) -> np.ndarray:

@@ -77,7 +77,12 @@ int ia_create(ia_ctx **out, const ia_species *species, const ia_trap *trap, doub
 typedef enum {
     IA_IC_EXPLICIT = 0, /* caller supplies y0[n][12] and phase[n]                                  */
     IA_IC_GRID = 1,     /* cell-centred uniform (theta,phi) grid, head-on (R1)      */
-    IA_IC_PHILOX = 2    /* Philox4x32-10(seed; index, cell) directions / phases / energies (R2)     */
+    IA_IC_PHILOX = 2,   /* Philox4x32-10(seed; index, cell) directions / phases / energies (R2)     */
+    IA_IC_THERMAL = 3   /* thermal run (R18): atom uniform on the r0 sphere with a
+                           Maxwell-Boltzmann velocity at T_atom_uK, negated if needed so that v_r < 0; ion
+                           position and velocity Gaussian at T_ion_uK in a harmonic trap of frequency
+                           |q_x| Omega_rf / 2^(3/2); normal deviates by Box-Muller on Philox blocks 2..6;
+                           rf phase as phase_mode says                                              */
 } ia_ic_mode;
 
 /* Launches of the cooperative kernel per straggler phase: a chain of levels, each lasting twice as long
@@ -114,6 +119,7 @@ typedef struct {
     uint32_t cell;         /* PHILOX counter word 2 (BASELINE.json configs[2]: Philox(seed,cell,index)) */
     uint64_t first_index;  /* global index of trajectory 0 (GRID: must be 0 <= first_index, the
                               grid position is first_index + j)                                     */
+    double T_atom_uK, T_ion_uK; /* THERMAL: bath and ion temperatures in microkelvin (> 0)         */
 } ia_launch;
 
 /* Per-trajectory outcome, 64 bytes, little-endian (R6, R7, R10). */
@@ -132,7 +138,8 @@ typedef struct {
 } ia_record;
 
 #define IA_HIST_BINS 32
-/* Ensemble reduction of one launch (R16), 512 bytes.  The library
+#define IA_LIFE_BINS 64
+/* Ensemble reduction of one launch (R16, R17), 1024 bytes.  The library
  * ACCUMULATES into it: the caller zeroes it before the first launch it should cover. */
 typedef struct {
     uint64_t n_done;            /* trajectories finished                                            */
@@ -149,6 +156,11 @@ typedef struct {
     uint64_t steps_coop;        /* attempted steps (incl. localisation) they took there              */
     uint64_t t_bulk_end_ns;     /* last %globaltimer over the warps of the bulk kernel               */
     uint64_t reserved[13];
+    /* Lifetimes of the complexes (n_coll >= 2), quarter-octave bins of q = t_life / T_rf (PAPER.md:34,40,
+     * Fig. 2: the fraction of complexes still alive after t is 1 - cumulative sum / n_complex; R17):
+     * bin b = clamp(ilogb(((q q) (q q))) + 8, 0, 63), products rounded separately, i.e. bin b holds
+     * 2^((b-8)/4) <= q < 2^((b-7)/4): from T_rf/4 in bin 0 to 13 777 T_rf and beyond in bin 63. */
+    uint64_t hist_tlife[IA_LIFE_BINS];
 } ia_summary;
 
 typedef struct {

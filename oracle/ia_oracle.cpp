@@ -371,6 +371,47 @@ int generate(const Derived &D, const oracle_gen &g, uint64_t index, double y0[12
             phi = 2.0 * PI * u2;
         }
         st = std::sqrt(1.0 - ct * ct);
+    } else if (g.mode == 3) {
+        /* THERMAL (reading R18).  Atom: uniform on the sphere of radius r0 about the trap
+         * centre, Cartesian velocity components Gaussian with variance k_B T/m_a, "negated if needed to enforce
+         * v_r < 0".  Ion: position and momentum Gaussian "corresponding to a fixed temperature ... for a spherical
+         * harmonic trap with frequency omega = q_x Omega_rf / 2^(3/2)".  Normal deviates by Box-Muller on the
+         * Philox blocks 2..6: (z_2k, z_2k+1) = sqrt(-2 ln u_a) (cos 2 pi u_b, sin 2 pi u_b). */
+        if (!(g.T_atom_uK > 0.0) || !(g.T_ion_uK > 0.0) || D.q[0] == 0.0) return -1;
+        ct = 2.0 * u1 - 1.0;
+        phi = 2.0 * PI * u2;
+        st = std::sqrt(1.0 - ct * ct);
+        double z[10];
+        for (uint32_t b = 2; b <= 6; ++b) {
+            uint32_t w[4];
+            ctr[3] = b;
+            philox(ctr, key, w);
+            const double ua = u53(w[0], w[1]), ub = u53(w[2], w[3]);
+            const double R = std::sqrt(-2.0 * std::log(ua));
+            z[2 * (b - 2)] = R * std::cos(2.0 * PI * ub);
+            z[2 * (b - 2) + 1] = R * std::sin(2.0 * PI * ub);
+        }
+        const double kT_i = g.T_ion_uK * 1e-6 * KB_EH_PER_K, kT_a = g.T_atom_uK * 1e-6 * KB_EH_PER_K;
+        const double w_h = std::fabs(D.q[0]) * D.Omega / std::pow(2.0, 1.5);
+        const double s_v = std::sqrt(kT_i / D.m_i), s_r = s_v / w_h, s_a = std::sqrt(kT_a / D.m_a);
+        const double n[3] = {st * std::cos(phi), st * std::sin(phi), ct};
+        double va[3], vr = 0.0;
+        for (int k = 0; k < 3; ++k) {
+            va[k] = s_a * z[6 + k];
+            vr += va[k] * n[k];
+        }
+        const double sign = (vr > 0.0) ? -1.0 : 1.0;
+        double v2 = 0.0;
+        for (int k = 0; k < 3; ++k) {
+            y0[k] = s_r * z[k];
+            y0[3 + k] = D.r0 * n[k];
+            y0[6 + k] = s_v * z[3 + k];
+            y0[9 + k] = sign * va[k];
+            v2 += va[k] * va[k];
+        }
+        *phase = (g.phase_mode == 1) ? 2.0 * PI * u3 : g.phase0;
+        *E_au = 0.5 * D.m_a * v2;
+        return 0;
     } else {
         return -1;
     }

@@ -44,13 +44,14 @@ typedef struct {
 
 /* initial-condition generator description (mirrors the launch descriptor of the boundary) */
 typedef struct {
-    int32_t mode;                 /* 1 = GRID, 2 = PHILOX (0 = explicit is not generated)  */
+    int32_t mode;                 /* 1 = GRID, 2 = PHILOX, 3 = THERMAL (0 = explicit is not generated) */
     int32_t domain;               /* 0 octant, 1 full sphere                              */
     int32_t phase_mode;           /* 0 fixed phase0, 1 uniform in [0,2pi) from Philox      */
     uint32_t n_theta, n_phi;      /* GRID                                                  */
     double phase0;
     double E_min_uK, E_max_uK;    /* equal: fixed energy; else log-uniform from Philox     */
     uint64_t seed; uint32_t cell; uint64_t first_index;
+    double T_atom_uK, T_ion_uK;   /* THERMAL (reading R18): bath and ion temperatures */
 } oracle_gen;
 
 int  oracle_derive(const oracle_params *p, oracle_derived *d);

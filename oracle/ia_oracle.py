@@ -64,7 +64,8 @@ class OracleGen(C.Structure):
     _fields_ = [("mode", C.c_int32), ("domain", C.c_int32), ("phase_mode", C.c_int32),
                 ("n_theta", C.c_uint32), ("n_phi", C.c_uint32), ("phase0", C.c_double),
                 ("E_min_uK", C.c_double), ("E_max_uK", C.c_double),
-                ("seed", C.c_uint64), ("cell", C.c_uint32), ("first_index", C.c_uint64)]
+                ("seed", C.c_uint64), ("cell", C.c_uint32), ("first_index", C.c_uint64),
+                ("T_atom_uK", C.c_double), ("T_ion_uK", C.c_double)]
 
 
 _lib = None
@@ -115,7 +116,8 @@ def to_params(p) -> OracleParams:
 def to_gen(l) -> OracleGen:
     """l: ia_inputs.Launch."""
     return OracleGen(l.mode, l.domain, l.phase_mode, l.n_theta, l.n_phi, l.phase0, l.E_min_uK, l.E_max_uK,
-                     l.seed, l.cell, l.first_index)
+                     l.seed, l.cell, l.first_index, float(getattr(l, "T_atom_uK", 0.0)),
+                     float(getattr(l, "T_ion_uK", 0.0)))
 
 
 def derive(p) -> dict:
@@ -223,3 +225,28 @@ def tableau():
     c, a, b, bh = np.empty(7), np.empty(49), np.empty(7), np.empty(7)
     lib().oracle_tableau(_dp(c), _dp(a), _dp(b), _dp(bh))
     return c, a.reshape(7, 7), b, bh
+
+
+# ---- reductions over the outcomes of an ensemble (plain numpy, the definitions written out) -------------
+
+def life_bins(t_life, n_coll, T_rf: float, nbins: int = 64) -> np.ndarray:
+    """Histogram of complex lifetimes (Fig. 2; reading R17): over trajectories with
+    n_coll >= 2, bin = clamp(ilogb(((q q)(q q))) + 8, 0, nbins-1) with q = t_life / T_rf, every product rounded
+    to double -- quarter-octave bins, bin b holding 2^((b-8)/4) <= q < 2^((b-7)/4)."""
+    t_life = np.asarray(t_life, dtype=np.float64)
+    sel = np.asarray(n_coll) >= 2
+    q = t_life[sel] / np.float64(T_rf)
+    q2 = q * q
+    q4 = q2 * q2
+    _, ex = np.frexp(q4)                      # q4 = m 2^ex with 0.5 <= m < 1, so ilogb(q4) = ex - 1
+    e = np.where(q4 > 0.0, ex - 1, -1023)
+    b = np.clip(e + 8, 0, nbins - 1).astype(np.int64)
+    return np.bincount(b, minlength=nbins).astype(np.uint64)
+
+
+def survival(t_life, n_coll, times) -> np.ndarray:
+    """Fraction of complexes (n_coll >= 2) still alive after each of `times` (Fig. 2)."""
+    t = np.asarray(t_life, dtype=np.float64)[np.asarray(n_coll) >= 2]
+    if len(t) == 0:
+        return np.zeros(len(times))
+    return np.array([(t > x).mean() for x in np.asarray(times, dtype=np.float64)])

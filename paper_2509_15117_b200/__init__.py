@@ -28,10 +28,11 @@ _HERE = Path(__file__).resolve().parent
 LIB_PATH = _HERE / "libia_b200.so"
 
 IA_OK, IA_EINVAL, IA_ENOMEM, IA_ECUDA, IA_EDEVICE = 0, -1, -2, -3, -4
-IA_IC_EXPLICIT, IA_IC_GRID, IA_IC_PHILOX = 0, 1, 2
+IA_IC_EXPLICIT, IA_IC_GRID, IA_IC_PHILOX, IA_IC_THERMAL = 0, 1, 2, 3
 IA_PATH_AUTO, IA_PATH_BULK_ONLY, IA_PATH_COOP_ONLY = 0, 1, 2
 IA_ARITH_NOFMA, IA_ARITH_FMA, IA_ARITH_FMA_COOP = 0, 1, 2
 IA_HIST_BINS = 32
+IA_LIFE_BINS = 64
 IA_STRAGGLER_LEVELS = 12
 
 # every symbol include/ia.h declares (tests/test_cabi.py checks the library exports each of them)
@@ -66,7 +67,8 @@ class ia_launch(C.Structure):
                 ("n_theta", C.c_uint32), ("n_phi", C.c_uint32), ("path", C.c_int32), ("n", C.c_uint64),
                 ("y0", C.c_void_p), ("phase", C.c_void_p), ("phase0", C.c_double),
                 ("E_min_uK", C.c_double), ("E_max_uK", C.c_double), ("seed", C.c_uint64),
-                ("cell", C.c_uint32), ("first_index", C.c_uint64)]
+                ("cell", C.c_uint32), ("first_index", C.c_uint64),
+                ("T_atom_uK", C.c_double), ("T_ion_uK", C.c_double)]
 
 
 class ia_outputs(C.Structure):
@@ -81,8 +83,8 @@ SUMMARY_DTYPE = np.dtype([("n_done", "<u8"), ("n_status", "<u8", (5,)), ("n_comp
                           ("sum_ke", "<f8"), ("sum_ke2", "<f8"), ("hist_ncoll", "<u8", (IA_HIST_BINS,)),
                           ("t_first_idle_ns", "<u8"), ("t_start_ns", "<u8"), ("t_end_ns", "<u8"),
                           ("warn", "<u8"), ("n_handoff", "<u8"), ("steps_coop", "<u8"), ("t_bulk_end_ns", "<u8"),
-                          ("reserved", "<u8", (13,))])
-RECORD_BYTES, SUMMARY_BYTES, IC_DUMP_COLS = 64, 512, 14
+                          ("reserved", "<u8", (13,)), ("hist_tlife", "<u8", (IA_LIFE_BINS,))])
+RECORD_BYTES, SUMMARY_BYTES, IC_DUMP_COLS = 64, 1024, 14
 assert RECORD_DTYPE.itemsize == RECORD_BYTES and SUMMARY_DTYPE.itemsize == SUMMARY_BYTES
 
 _lib: Optional[C.CDLL] = None
@@ -180,6 +182,7 @@ def make_launch(launch, y0=None, phase=None) -> ia_launch:
     L.y0, L.phase = _ptr(y0), _ptr(phase)
     L.phase0, L.E_min_uK, L.E_max_uK = float(launch.phase0), float(launch.E_min_uK), float(launch.E_max_uK)
     L.seed, L.cell, L.first_index = int(launch.seed), int(launch.cell), int(launch.first_index)
+    L.T_atom_uK, L.T_ion_uK = float(getattr(launch, "T_atom_uK", 0.0)), float(getattr(launch, "T_ion_uK", 0.0))
     return L
 
 
@@ -202,7 +205,7 @@ def ia_destroy(handle) -> None:
 
 def ia_run(handle, launch: ia_launch, records=None, summary=None, ic_dump=None, stream=None) -> None:
     """Asynchronous: enqueues on `stream` (default: torch's current stream).  All buffers are device
-    tensors: records uint8 [n*64], summary uint8 [512] (accumulated into), ic_dump float64 [n,14]."""
+    tensors: records uint8 [n*64], summary uint8 [1024] (accumulated into), ic_dump float64 [n,14]."""
     out = ia_outputs(_ptr(records), _ptr(summary), _ptr(ic_dump))
     _check(load().ia_run(handle, C.byref(launch), C.byref(out), _stream_handle(stream)), handle)
 
@@ -359,7 +362,7 @@ class Context:
         ia_wait(self.handle)
 
     def alloc(self, n: int, ic_dump: bool = False):
-        """(records uint8[n*64], summary uint8[512] zeroed, ic_dump float64[n,14] or None) on the device."""
+        """(records uint8[n*64], summary uint8[1024] zeroed, ic_dump float64[n,14] or None) on the device."""
         import torch
         dev = torch.device("cuda", self.device)
         rec = torch.empty(max(n, 1) * RECORD_BYTES, dtype=torch.uint8, device=dev)

@@ -80,6 +80,7 @@ struct ia_ctx {
     unsigned counter_next = 0;
     size_t queue_cap = 0; /* hand-over entries ONE run can produce: one per lane of a full bulk grid */
     int handoff_lanes = 16;
+    double w_harm = 0.0;                   /* |q_x| Omega / 2^(3/2): the ion's trap frequency in thermal runs */
     int levels = IA_STRAGGLER_LEVELS;      /* launches of the straggler chain (ia_set_chain) */
     unsigned level_budget = 8192u;         /* iterations of its first level after the queue ran dry */
     int n_sm = 0;
@@ -186,12 +187,17 @@ int ia_create(ia_ctx **out, const ia_species *sp, const ia_trap *tr, double De_K
     P.r_e = std::pow(2.0 * P.C8 / P.C4, 0.25);
     P.c8x8 = 8.0 * P.C8;
     P.neg_c4x4 = -4.0 * P.C4;
+    P.c8_a = P.c8x8 / P.m_a;
+    P.c4_a = P.neg_c4x4 / P.m_a;
+    P.c8_i = -P.c8x8 / P.m_i;
+    P.c4_i = -P.neg_c4x4 / P.m_i;
     P.omega = tr->omega_rf_au;
     P.T_rf = 2.0 * PI / P.omega;
     for (int k = 0; k < 3; ++k) {
         P.ka[k] = -tr->a[k] * (P.omega * P.omega / 4.0);
         P.kq[k] = -2.0 * tr->q[k] * (P.omega * P.omega / 4.0);
     }
+    c->w_harm = std::fabs(tr->q[0]) * P.omega / std::pow(2.0, 1.5);
     P.rtol = T.rtol;
     P.atol = T.atol;
     P.thr = T.atol / T.rtol;
@@ -333,7 +339,7 @@ static int make_gen(ia_ctx *ctx, const ia_launch *L, IaGen *G, unsigned long lon
     if (!L) return fail_inval(ctx, "launch is NULL");
     std::memset(G, 0, sizeof(*G));
     *warn = 0;
-    if (L->mode != IA_IC_EXPLICIT && L->mode != IA_IC_GRID && L->mode != IA_IC_PHILOX)
+    if (L->mode != IA_IC_EXPLICIT && L->mode != IA_IC_GRID && L->mode != IA_IC_PHILOX && L->mode != IA_IC_THERMAL)
         return fail_inval(ctx, "launch.mode is not an ia_ic_mode");
     if (L->path != IA_PATH_AUTO && L->path != IA_PATH_BULK_ONLY && L->path != IA_PATH_COOP_ONLY)
         return fail_inval(ctx, "launch.path is not an ia_path");
@@ -349,6 +355,26 @@ static int make_gen(ia_ctx *ctx, const ia_launch *L, IaGen *G, unsigned long lon
     if (L->domain != 0 && L->domain != 1) return fail_inval(ctx, "launch.domain must be 0 or 1");
     if (L->phase_mode != 0 && L->phase_mode != 1) return fail_inval(ctx, "launch.phase_mode must be 0 or 1");
     if (!std::isfinite(L->phase0)) return fail_inval(ctx, "launch.phase0 is not finite");
+    if (L->mode == IA_IC_THERMAL) {
+        /* a1 for a thermal run: widths of the ion's and the atom's Gaussians */
+        if (!(std::isfinite(L->T_atom_uK) && L->T_atom_uK > 0.0 && std::isfinite(L->T_ion_uK) && L->T_ion_uK > 0.0))
+            return fail_inval(ctx, "THERMAL launch needs T_atom_uK > 0 and T_ion_uK > 0");
+        if (L->domain != 1) return fail_inval(ctx, "THERMAL launch starts on the full sphere: domain must be 1");
+        const double w_h = ctx->w_harm;
+        if (!(w_h > 0.0)) return fail_inval(ctx, "THERMAL launch needs q_x != 0 (ion trap frequency |q_x| Omega / 2^(3/2))");
+        const double kT_i = L->T_ion_uK * 1e-6 * KB_EH_PER_K, kT_a = L->T_atom_uK * 1e-6 * KB_EH_PER_K;
+        G->domain = 1;
+        G->phase_mode = L->phase_mode;
+        G->phase0 = L->phase0;
+        G->seed = L->seed;
+        G->cell = L->cell;
+        G->theta_span_pi = 1.0;
+        G->phi_span_pi = 2.0;
+        G->sig_v_ion = std::sqrt(kT_i / ctx->P.m_i);
+        G->sig_r_ion = G->sig_v_ion / w_h;
+        G->sig_v_atom = std::sqrt(kT_a / ctx->P.m_a);
+        return IA_OK;
+    }
     if (!(std::isfinite(L->E_min_uK) && L->E_min_uK > 0.0 && std::isfinite(L->E_max_uK) && L->E_max_uK >= L->E_min_uK))
         return fail_inval(ctx, "need 0 < E_min_uK <= E_max_uK");
     G->domain = L->domain;
@@ -548,7 +574,7 @@ static int submit_host_impl(ia_ctx *ctx, const ia_launch *launch, const ia_outpu
     const int g = (handoff && ctx->depth > 0) ? ctx->cur : 0;
     IaGeneration &G = ctx->gen[g];
     const int k = handoff ? G.n_pending : 0;
-    /* staging layout: [summary 512][records n*64][ic_dump n*14*8][y0 n*12*8][phase n*8] */
+    /* staging layout: [summary 1024][records n*64][ic_dump n*14*8][y0 n*12*8][phase n*8] */
     const size_t off_rec = sizeof(ia_summary);
     const size_t off_ic = off_rec + (host_out->records ? n * sizeof(ia_record) : 0);
     const size_t off_y0 = off_ic + (host_out->ic_dump ? n * 14 * sizeof(double) : 0);

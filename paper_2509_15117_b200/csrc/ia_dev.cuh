@@ -74,6 +74,9 @@ struct IaParams {
     double neg_inv_m_i; /* -1/m_i                       */
     double m_i, m_a;
     double c8x8, neg_c4x4; /* 8 C8, -4 C4              */
+    /* the same with the masses folded in: acceleration = u^3 (c8 u^2 + c4) d,  u = 1/r^2 */
+    double c8_a, c4_a;     /*  8 C8/m_a, -4 C4/m_a (atom) */
+    double c8_i, c4_i;     /* -8 C8/m_i,  4 C4/m_i (ion)  */
     /* trap: A_i,k += (ka_k + kq_k cos(Omega t + phase)) r_i,k */
     double ka[3];       /* -a_k Omega^2/4               */
     double kq[3];       /* -q_k Omega^2/2               */
@@ -112,7 +115,10 @@ IA_DEV double ia_rcp(double x) {
 
 /* x^(-1/5) for x in [1e-30, 1e30]: FP32 MUFU seed (lg2/ex2, rel. err ~1e-6) and one Newton step
  * y <- y (6 - x y^5)/5 (rel. err -> 3 e^2 ~ 3e-12).  The result only scales the next step size: a relative
- * 3e-12 there moves the next step's error estimate by 1.5e-11 of itself, far below its own rounding. */
+ * 3e-12 there moves the next step's error estimate by 1.5e-11 of itself, far below its own rounding.
+ * (A variant without the double-precision reciprocal in front of it -- Newton on den - num y^5 with an FP32
+ * divisor -- shortens the straggler kernel's step by 5 % and lengthens the bulk kernel's by 5 %: measured,
+ * profiles/r01d; the two kernels must run the same arithmetic, so it stays out.) */
 IA_DEV double ia_inv_fifth_root(double x) {
     const float xf = (float)x;
     float lf;
@@ -233,8 +239,8 @@ IA_DEV double ia_dot3(const double (&a)[3], const double (&b)[3]) {
 /* ---- right-hand side (reading O1) ------------------------------------------------ */
 
 /* Accelerations of the local axes at positions (Xi, Xa), with c = cos(Omega t + phase).
- * Also returns the gathered separation d = r_a - r_i, r^2 = |d|^2 and s = u^3 (8 C8 u^2 - 4 C4),
- * u = 1/r^2: force on the atom = -dV/dr d/r = s d. */
+ * Also returns the gathered separation d = r_a - r_i, r^2 = |d|^2 and s = u^3 (8 C8 u^2 - 4 C4)/m_a,
+ * u = 1/r^2: acceleration of the atom = -(dV/dr) d/(r m_a) = s d. */
 template <int LPT, bool FUSED>
 IA_DEV void ia_accel(const IaParams &P, const IaLane<LPT> &L, const double (&Xi)[3 / LPT], const double (&Xa)[3 / LPT],
                      double c, double (&Ai)[3 / LPT], double (&Aa)[3 / LPT], double (&D)[3], double &r2, double &s) {
@@ -246,10 +252,14 @@ IA_DEV void ia_accel(const IaParams &P, const IaLane<LPT> &L, const double (&Xi)
     r2 = ia_dot3<FUSED>(D, D);
     const double u = ia_rcp(r2);
     const double u2 = u * u;
-    const double t = ia_fma<FUSED>(P.c8x8, u2, P.neg_c4x4);
-    s = (u2 * u) * t;
-    const double sa = s * P.inv_m_a;
-    const double si = s * P.neg_inv_m_i;
+    /* s/m for each particle straight from u: two independent fma and two products (one operation less on the
+     * dependent chain r^2 -> force than forming s first and scaling it by 1/m) */
+    const double ta = ia_fma<FUSED>(P.c8_a, u2, P.c4_a);
+    const double ti = ia_fma<FUSED>(P.c8_i, u2, P.c4_i);
+    const double u3 = u2 * u;
+    const double sa = u3 * ta;
+    const double si = u3 * ti;
+    s = sa; /* NaN whenever r2 is 0, inf or NaN */
 #pragma unroll
     for (int a = 0; a < NA; ++a) {
         Aa[a] = sa * d[a];

@@ -73,6 +73,36 @@ __device__ __forceinline__ void ia_generate_ic(const IaParams &P, const IaGen &G
     const double u1 = ia_u53(w0[0], w0[1]), u2 = ia_u53(w0[2], w0[3]);
     const double u3 = ia_u53(w1[0], w1[1]), u4 = ia_u53(w1[2], w1[3]);
     double ct, st, sp, cp;
+    if (G.mode == IA_IC_THERMAL) {
+        /* thermal run (reading R18): atom uniform on the r0 sphere, Maxwell-Boltzmann velocity
+         * negated if needed so that v_r < 0; ion Gaussian in position and velocity.  Normal deviates by
+         * Box-Muller on Philox blocks 2..6: (z_2k, z_2k+1) = sqrt(-2 ln u_a) (cos 2 pi u_b, sin 2 pi u_b). */
+        ct = 2.0 * u1 - 1.0;
+        st = sqrt(1.0 - ct * ct);
+        sincospi(2.0 * u2, &sp, &cp);
+        double z[10];
+#pragma unroll
+        for (unsigned b = 2; b <= 6; ++b) {
+            unsigned w[4];
+            ia_philox((unsigned)gi, (unsigned)(gi >> 32), G.cell, b, (unsigned)G.seed, (unsigned)(G.seed >> 32), w);
+            const double R = sqrt(-2.0 * log(ia_u53(w[0], w[1])));
+            double sb, cb;
+            sincospi(2.0 * ia_u53(w[2], w[3]), &sb, &cb);
+            z[2 * (b - 2)] = R * cb;
+            z[2 * (b - 2) + 1] = R * sb;
+        }
+        const double n0 = st * cp, n1 = st * sp, n2 = ct;
+        double va0 = G.sig_v_atom * z[6], va1 = G.sig_v_atom * z[7], va2 = G.sig_v_atom * z[8];
+        const double vr = va0 * n0 + va1 * n1 + va2 * n2;
+        const double sign = (vr > 0.0) ? -1.0 : 1.0;
+        ic->E_au = 0.5 * P.m_a * (va0 * va0 + va1 * va1 + va2 * va2);
+        ic->x[0] = G.sig_r_ion * z[0]; ic->x[1] = G.sig_r_ion * z[1]; ic->x[2] = G.sig_r_ion * z[2];
+        ic->v[0] = G.sig_v_ion * z[3]; ic->v[1] = G.sig_v_ion * z[4]; ic->v[2] = G.sig_v_ion * z[5];
+        ic->x[3] = P.r0 * n0; ic->x[4] = P.r0 * n1; ic->x[5] = P.r0 * n2;
+        ic->v[3] = sign * va0; ic->v[4] = sign * va1; ic->v[5] = sign * va2;
+        ic->phase = (G.phase_mode == 1) ? 6.28318530717958647692 * u3 : G.phase0;
+        return;
+    }
     if (G.mode == IA_IC_GRID) {
         const unsigned long long ii = gi / G.n_phi, jj = gi % G.n_phi;
         /* theta = (i + 1/2) span / n_theta, evaluated as sincospi(theta/pi) */
@@ -166,7 +196,7 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
         ia_record *rec[IA_THREADS];   /* outputs of the run the group's trajectory belongs to */
         ia_summary *sum[IA_THREADS];
         unsigned steps_in[IA_THREADS], n_coll[IA_THREADS], n_tp[IA_THREADS], n_loc[IA_THREADS], steps_rej[IA_THREADS],
-            cnt[IA_THREADS];
+            cnt[IA_THREADS], wexh[IA_THREADS];
     } sh;
     double &t_first = sh.t_first[threadIdx.x], &t_last = sh.t_last[threadIdx.x], &phase = sh.phase[threadIdx.x],
            &s_old = sh.s_old[threadIdx.x];
@@ -182,7 +212,8 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
     t_first = 0.0; t_last = 0.0; slot = 0; steps_in = 0; n_coll = 0; n_tp = 0; n_loc = 0; steps_rej = 0;
     int mode = MODE_IDLE;
     bool failed = false;
-    bool wexh = false; /* warp-uniform: the work counter is empty */
+    unsigned &wexh = sh.wexh[threadIdx.x]; /* warp-uniform flag: the work counter is empty */
+    wexh = 0u;
     ia_park<LPT>(L, Y);
     if (!RESUME && O.summary != nullptr && threadIdx.x == 0) {
         const unsigned long long t0 = ia_globaltimer();
@@ -202,7 +233,7 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
     bool first_refill = resume;
 
     for (;;) {
-        const bool was_exh = wexh;
+        const bool was_exh = wexh != 0u;
         /* ---- refill idle groups from the global work counter (a12) ---- */
         const bool want = L.valid && (mode == MODE_IDLE) && !wexh;
         const unsigned wm = __ballot_sync(IA_FULL, want && L.leader);
@@ -221,7 +252,7 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
             if (__any_sync(IA_FULL, want && !got)) {
                 if (!wexh && O.summary != nullptr && !resume && lane == 0)
                     atomicCAS((unsigned long long *)&O.summary->t_first_idle_ns, 0ull, ia_globaltimer());
-                wexh = true;
+                wexh = 1u;
             }
             if (got) {
                 if (resume) {
@@ -326,7 +357,7 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
             unsigned long long c = 0;
             if (lane == 0) c = IA_DEALT + *(volatile unsigned long long *)S.counter;
             c = __shfl_sync(IA_FULL, c, 0);
-            if (c >= IA_N_TOTAL) wexh = true;
+            if (c >= IA_N_TOTAL) wexh = 1u;
         }
         if (wexh && !was_exh) cnt = 0u;
 
@@ -389,8 +420,9 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
 
         /* ---- controller, events, termination: straight-line selects; rare cases branch ---- */
         const double hs = h; /* the step just attempted */
-        const bool accept = so.finite && (so.err.num <= P.rtol * so.err.den);
-        double xr = so.err.num * ia_rcp(so.err.den * P.rtol); /* err / rtol */
+        const double denr = P.rtol * so.err.den;
+        const bool accept = so.finite && (so.err.num <= denr);
+        double xr = so.err.num * ia_rcp(denr); /* err / rtol */
         xr = so.finite ? xr : 1e30;
         xr = ia_max(ia_min(xr, 1e30), 1e-30); /* NaN -> 1e30 (ia_min returns its second operand then) */
         const double fac = 0.8 * ia_inv_fifth_root(xr); /* 0.8 (rtol/err)^(1/5) */
@@ -520,6 +552,13 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
                         }
                         const int bin = (n_coll == 0u) ? 0 : min(32 - __clz(n_coll), IA_HIST_BINS - 1);
                         atomicAdd((unsigned long long *)&Sm->hist_ncoll[bin], 1ull);
+                        if (n_coll >= 2u) { /* lifetime of the complex, quarter-octave bins of t_life / T_rf (R17) */
+                            const double q = (t_last - t_first) / P.T_rf;
+                            const double q2 = q * q;
+                            const double q4 = q2 * q2;
+                            const int e = ((__double2hiint(q4) >> 20) & 0x7ff) - 1023;
+                            atomicAdd((unsigned long long *)&Sm->hist_tlife[max(0, min(e + 8, IA_LIFE_BINS - 1))], 1ull);
+                        }
                     }
                 }
                 mode = MODE_IDLE;

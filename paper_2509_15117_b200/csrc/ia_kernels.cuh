@@ -19,6 +19,7 @@ struct IaGen {
     double E_min_uK, log_E_ratio; /* E_uK = E_min exp(u4 log(E_max/E_min)); log_E_ratio = 0 -> fixed */
     double E_fixed_au, v0_fixed;  /* fixed-energy case, computed on the host                        */
     double theta_span_pi, phi_span_pi; /* angular spans in units of pi: 0.5/0.5 octant, 1/2 sphere   */
+    double sig_r_ion, sig_v_ion, sig_v_atom; /* THERMAL: sqrt(kT_i/m_i)/w_h, sqrt(kT_i/m_i), sqrt(kT_a/m_a) */
 };
 
 struct IaOut {

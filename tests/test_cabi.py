@@ -28,12 +28,13 @@ def test_header_symbols_are_all_exported():
 
 
 def test_struct_sizes_match_the_header():
-    # the byte layouts include/ia.h promises: 64-byte records, 512-byte summary
-    assert P.RECORD_DTYPE.itemsize == 64 and P.SUMMARY_DTYPE.itemsize == 512
+    # the byte layouts include/ia.h promises: 64-byte records, 1024-byte summary
+    assert P.RECORD_DTYPE.itemsize == 64 and P.SUMMARY_DTYPE.itemsize == 1024
     assert C.sizeof(P.ia_species) == 24 and C.sizeof(P.ia_trap) == 56 and C.sizeof(P.ia_tol) == 48
-    assert C.sizeof(P.ia_launch) == 96 and C.sizeof(P.ia_outputs) == 24
+    assert C.sizeof(P.ia_launch) == 112 and C.sizeof(P.ia_outputs) == 24
     assert P.RECORD_DTYPE.fields["va_f"][1] == 24 and P.RECORD_DTYPE.fields["status"][1] == 62
     assert P.SUMMARY_DTYPE.fields["hist_ncoll"][1] == 96 and P.SUMMARY_DTYPE.fields["warn"][1] == 376
+    assert P.SUMMARY_DTYPE.fields["hist_tlife"][1] == 512
 
 
 def test_strerror_and_null_arguments():

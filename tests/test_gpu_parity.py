@@ -335,7 +335,19 @@ def _ensemble_checks(rec, ref, label):
     print(f"\n{label}: n={n}  P(complex) gpu {k_g / n:.4f} oracle {k_o / len(ref):.4f} (diff {dp:+.4f}, 99% half-width {half:.4f}); "
           f"mean ke_ion diff {dm:+.3e} CI [{ci[0]:+.3e},{ci[1]:+.3e}]; median ke_ion gpu {med_g:.4e} oracle {med_o:.4e}; "
           f"hist gpu {S.ncoll_bins(rec['n_coll'])[:10]} oracle {S.ncoll_bins(ref['n_coll'])[:10]}")
-    return ok_p and ok_m and ok_h, (ok_p, ok_m, ok_h, bad)
+    # survival of the complexes (Fig. 2): fraction still alive after 5, 20 and 80 rf periods
+    ok_s = True
+    surv = []
+    if k_g >= 20 and k_o >= 20:
+        T = 2.067068666759e10
+        for x in (5.0, 20.0, 80.0):
+            a_g = int(((rec["n_coll"] >= 2) & (rec["t_life"] > x * T)).sum())
+            a_o = int(((ref["n_coll"] >= 2) & (ref["t_life"] > x * T)).sum())
+            ok_x, d_x, half_x = S.two_proportion_ok(a_g, k_g, a_o, k_o)
+            ok_s = ok_s and ok_x
+            surv.append(f"S({x:g} T_rf) gpu {a_g / k_g:.3f} oracle {a_o / k_o:.3f}")
+        print("   " + "; ".join(surv))
+    return ok_p and ok_m and ok_h and ok_s, (ok_p, ok_m, ok_h, ok_s, bad)
 
 
 def test_config1_subgrid_ensemble_and_regular_region(P):
@@ -357,8 +369,55 @@ def test_config1_subgrid_ensemble_and_regular_region(P):
     assert int(summ["n_done"]) == cell.launch.n
     assert int(summ["n_complex"]) == int((rec["n_coll"] >= 2).sum())
     assert np.array_equal(summ["hist_ncoll"], S.ncoll_bins(rec["n_coll"]).astype(np.uint64))
+    # lifetime histogram (R17): the device's bins of its own t_life, bit for bit against the oracle's binning
+    T_rf = O.derive(cell.params)["T_rf"]
+    assert np.array_equal(summ["hist_tlife"], O.life_bins(rec["t_life"], rec["n_coll"], T_rf))
+    assert int(summ["hist_tlife"].sum()) == int(summ["n_complex"]) > 1000
     esc = rec["status"] == 0
     assert abs(summ["sum_ke"] - rec["ke_ion"][esc].sum()) <= 1e-11 * rec["ke_ion"][esc].sum()
+
+
+def test_config1_full_grid_in_the_bench_configuration(P):
+    """BASELINE.json configs[1] at its full size (512x512 = 262,144 trajectories, t_max = 1e4 T_rf) the way bench.py
+    runs it: two passes of one generation (ia_set_pipeline), one straggler chain, joined.  The two passes give
+    bit-identical records; every 8th grid point in theta and phi (4,096 trajectories) is recomputed by the
+    oracle: per trajectory in the regular region, as an ensemble elsewhere; the summary adds up over the grid."""
+    import torch
+    cell = I.config1(512)
+    n = cell.launch.n
+    idx = I.subgrid_indices(512, 8)
+    with P.Context(cell.params) as ctx:
+        ctx.set_pipeline(2)
+        bufs = [ctx.alloc(n) for _ in range(2)]
+        for rec_d, summ_d, _ in bufs:
+            ctx.run(cell.launch, records=rec_d, summary=summ_d)
+        ctx.join()
+        torch.cuda.synchronize()
+        rec = P.view_records(bufs[0][0], n)
+        summ = P.view_summary(bufs[0][1])
+        _assert_records_identical(rec, P.view_records(bufs[1][0], n))
+        t = ctx.timing(0)
+        assert t["bulk_ms"] > 0.0 and t["coop_ms"] > 0.0
+    ref = O.run_generated(cell.params, cell.launch, indices=idx, nthreads=NTHREADS)
+    got = rec[idx]
+    ok, detail = _ensemble_checks(got, ref, "config1 512x512, every 8th point")
+    assert ok, detail
+    reg = (ref["n_coll"] == 1) & (got["n_coll"] == 1) & (ref["status"] == 0)
+    assert reg.sum() > 500
+    same, e_t, e_dir, e_v, e_k = _compare_regular(got[reg], ref[reg], "config1 512x512 regular region")
+    assert same.mean() >= 0.97
+    assert np.median(e_t[same]) <= 1e-8 and np.median(e_dir[same]) <= 1e-8
+    # properties that hold at any size
+    assert int(summ["n_done"]) == n and int(summ["n_status"].sum()) == n
+    assert int(summ["n_complex"]) == int((rec["n_coll"] >= 2).sum())
+    assert np.array_equal(summ["hist_ncoll"], S.ncoll_bins(rec["n_coll"]).astype(np.uint64))
+    assert int(summ["steps_acc"]) == int(rec["steps_acc"].astype(np.int64).sum())
+    assert np.array_equal(summ["hist_tlife"], O.life_bins(rec["t_life"], rec["n_coll"], O.derive(cell.params)["T_rf"]))
+    assert int(summ["n_handoff"]) > 0 and int(summ["steps_coop"]) > 0
+    esc = rec["status"] == 0
+    assert abs(summ["sum_ke"] - rec["ke_ion"][esc].sum()) <= 1e-10 * rec["ke_ion"][esc].sum()
+    assert np.all(rec["status"] <= 1) and (rec["status"] == 1).sum() < 100     # a few complexes outlive t_max
+    assert np.all(rec["n_coll"][rec["status"] == 0] >= 1)                      # head-on: every escape bounced once
 
 
 @pytest.mark.parametrize("which,ci", [("config2", 18), ("config2", 2), ("config3", 7), ("config4", 0)])
@@ -381,3 +440,44 @@ def test_philox_cells_ensemble(P, which, ci):
     assert ok, detail
     # trajectories still bound at t_max (status 1) are rare and agree as a proportion
     assert S.two_proportion_ok(int((rec["status"] != 0).sum()), n, int((ref["status"] != 0).sum()), n)[0]
+
+
+# ---------------------------------------------------------------------------------------------
+# thermal runs (reading R18)
+# ---------------------------------------------------------------------------------------------
+def test_thermal_generator_matches_oracle(P):
+    cell = I.thermal("Rb87", 3.0, n=3000)
+    launch = replace(cell.launch, first_index=(1 << 32) - 1500)     # the index carries into counter word 1
+    with P.Context(cell.params) as ctx:
+        ic = ctx.generate(launch)
+    y0, ph, E = O.generate(cell.params, launch, np.arange(3000))
+    assert np.array_equal(ic[:, 12], ph)                            # 2 pi u3: the same product on both sides
+    # Box-Muller through log / sqrt / sincospi on the device, log / sqrt / sin / cos of a rounded product on the
+    # host: a few ulp of each column's scale; the v_r < 0 negation must take the same branch everywhere
+    scale = np.abs(y0).max(axis=0)
+    assert np.max(np.abs(ic[:, :12] - y0) / scale) < 2e-15
+    assert np.max(np.abs(ic[:, 13] - E) / E) < 1e-14
+    assert np.all(np.sum(ic[:, 3:6] * ic[:, 9:12], axis=1) <= 0.0)
+    assert np.max(np.abs(np.linalg.norm(ic[:, 3:6], axis=1) - cell.params.r0_a0)) < 1e-9
+
+
+def test_thermal_run_ensemble(P):
+    """One bar of Fig. 3 in small: Yb+ + 87Rb at 1 uK bath temperature, 4,096 trajectories, the ICs the device
+    generated re-integrated by the oracle: ensemble statistics within the 99 % intervals, per-trajectory parity
+    where both sides see at most one bounce (trajectories that miss the ion included), counts add up."""
+    cell = I.thermal("Rb87", 1.0, n=4096)
+    cell = replace(cell, params=replace(cell.params, t_max_rf=2000.0))
+    with P.Context(cell.params) as ctx:
+        rec, summ, ic = ctx.run_sync(cell.launch, want_ic=True)
+    ref = O.run_explicit(cell.params, ic[:, :12], ic[:, 12], nthreads=NTHREADS)
+    ok, detail = _ensemble_checks(rec, ref, "thermal Rb87 1 uK")
+    assert ok, detail
+    assert np.array_equal(rec["status"] <= 1, np.ones(len(rec), dtype=bool))
+    reg = (ref["n_coll"] <= 1) & (rec["n_coll"] <= 1) & (ref["status"] == 0) & (rec["status"] == 0)
+    assert reg.sum() > 1000 and (ref["n_coll"] == 0).sum() > 100            # many atoms never reach short range
+    same, e_t, e_dir, e_v, e_k = _compare_regular(rec[reg], ref[reg], "thermal regular trajectories")
+    assert same.mean() >= 0.95
+    assert np.median(e_t[same]) <= 1e-8 and np.median(e_dir[same]) <= 1e-8
+    assert int(summ["n_done"]) == cell.launch.n
+    assert int(summ["n_complex"]) == int((rec["n_coll"] >= 2).sum())
+    assert np.array_equal(summ["hist_ncoll"], S.ncoll_bins(rec["n_coll"]).astype(np.uint64))

@@ -96,6 +96,35 @@ def test_device_cosine_polynomial_is_accurate_to_half_an_ulp():
     assert c[0] == 1
 
 
+def test_observables_formatting_on_constructed_records():
+    """observables.py is array arithmetic on records: back-scattering gives chi = pi and q = 2 m v, a 90 degree
+    deflection chi = pi/2 and q = sqrt(2) m v, forward flight zero; the survival curve of a known histogram and the
+    slope of an exact power law come back."""
+    import paper_2509_15117_b200 as P
+    from paper_2509_15117_b200 import observables as Ob
+    v, m = 1.0e-8, 158425.415
+    ic = np.zeros((4, 14)); ic[:, 9] = -v
+    rec = np.zeros(4, dtype=P.RECORD_DTYPE)
+    rec["va_f"] = [[v, 0, 0], [0, v, 0], [-v, 0, 0], [0, 0, -2 * v]]
+    rec["n_coll"] = [1, 100, 1, 3]
+    chi, q = Ob.scattering(rec, ic, m)
+    assert np.allclose(chi, [np.pi, np.pi / 2, 0.0, np.pi / 2], atol=1e-15)
+    assert np.allclose(q, [2 * m * v, np.sqrt(2) * m * v, 0.0, np.sqrt(5) * m * v], rtol=1e-15)
+    mp = Ob.maps(rec, ic, m, 2, 2)
+    assert mp["log10_bounces"].tolist() == [[0.0, 2.0], [0.0, np.log10(3.0)]]
+    assert mp["complex"].tolist() == [[False, True], [False, True]]
+    assert mp["momentum_transfer_clipped"].max() <= Ob.Q_CLIP_AU
+    T = 2.0e10
+    summ = np.zeros(1, dtype=P.SUMMARY_DTYPE)[0]
+    h = np.zeros(P.IA_LIFE_BINS, dtype=np.uint64); h[8] = 2; h[12] = 1; h[16] = 1      # q in [1,2^.25), [2,..), [4,..)
+    summ["hist_tlife"] = h
+    t, S = Ob.survival_curve(summ, T)
+    assert len(t) == P.IA_LIFE_BINS - 1 and t[7] == T and t[11] == 2 * T
+    assert S[6] == 1.0 and S[7] == 1.0 and S[8] == 0.5 and S[11] == 0.5 and S[12] == 0.25 and S[16] == 0.0
+    tt = T * 2.0 ** np.arange(0, 10)
+    assert abs(Ob.power_law_exponent(tt, 3.0 * tt ** -1.5, t_min=2 * T) + 1.5) < 1e-12
+
+
 def test_config_recipes_match_baseline_json():
     import json
     cfg = json.load(open(os.path.join(ROOT, "BASELINE.json")))["configs"]

@@ -498,3 +498,68 @@ def test_heavy_cold_atoms_form_complexes_and_light_hot_ones_do_not():
     # complexes have a positive lifetime, and first/last collision times are ordered
     cx = cold[cold["n_coll"] >= 2]
     assert np.all(cx["t_life"] > 0) and np.all(cx["t_last"] > cx["t_first"])
+
+
+def test_lifetime_bins_are_quarter_octaves():
+    """R17: the lifetime histogram's bin index against the plain definition floor(4 log2(t_life/T_rf)) + 8 away
+    from the bin edges, at exact powers of two (bin 4k + 8, lower edge inclusive), and its clamps."""
+    T = O.derive(I.config1(8).params)["T_rf"]
+    rng = np.random.default_rng(7)
+    q = 2.0 ** rng.uniform(-1.9, 13.7, 5000)
+    frac = (4 * np.log2(q)) % 1.0
+    q = q[(frac > 1e-6) & (frac < 1 - 1e-6)]
+    for x in q[:2000]:
+        h = O.life_bins([x * T], [2], T)
+        assert h.sum() == 1 and h[int(np.floor(4 * np.log2(x))) + 8] == 1
+    for k in range(-2, 14):
+        assert O.life_bins([2.0 ** k * T], [5], T)[4 * k + 8] == 1
+        assert O.life_bins([2.0 ** k * (1.0 - 1e-12) * T], [5], T)[max(4 * k + 7, 0)] == 1
+    assert O.life_bins([1e-9 * T, 0.0, 1e9 * T], [2, 2, 2], T)[[0, 63]].tolist() == [2, 1]
+    assert O.life_bins([3.0 * T, 3.0 * T], [1, 0], T).sum() == 0                  # not complexes
+    s = O.survival(np.array([1.0, 2.0, 3.0, 4.0, 9.0]), np.array([2, 2, 3, 9, 1]), [0.5, 2.0, 3.5, 10.0])
+    assert s.tolist() == [1.0, 0.5, 0.25, 0.0]
+
+
+def test_thermal_generator_distributions():
+    """Reading R18: the thermal-run generator against what the text fixes.  Atom uniform on the
+    r0 sphere, Maxwell-Boltzmann velocity with v_r < 0 enforced by negation (so the radial component is half-normal
+    and the tangential ones normal); ion position and velocity Gaussian for a harmonic trap of frequency
+    q_x Omega / 2^(3/2) at 10 uK -- which is the lowest-order secular frequency (1/2) Omega sqrt(a + q^2/2) at a = 0."""
+    from scipy import stats
+    n = 40000
+    c = I.thermal("Rb87", 3.0, n=n)
+    y0, ph, E = O.generate(c.params, c.launch, np.arange(n))
+    d = O.derive(c.params)
+    kB = 3.1668115634564e-6
+    kT_a, kT_i = 3.0e-6 * kB, 10.0e-6 * kB
+    r_a, v_a, r_i, v_i = y0[:, 3:6], y0[:, 9:12], y0[:, 0:3], y0[:, 6:9]
+    rn = np.linalg.norm(r_a, axis=1)
+    assert np.max(np.abs(rn - c.params.r0_a0)) < 1e-9
+    nhat = r_a / rn[:, None]
+    # uniform on the sphere: cos(theta) uniform on [-1,1], phi uniform on [0, 2 pi)
+    assert stats.kstest((nhat[:, 2] + 1) / 2, "uniform").pvalue > 1e-3
+    assert stats.kstest(np.mod(np.arctan2(nhat[:, 1], nhat[:, 0]), 2 * np.pi) / (2 * np.pi), "uniform").pvalue > 1e-3
+    assert stats.kstest(ph / (2 * np.pi), "uniform").pvalue > 1e-3
+    # atom velocity: inward, radial part half-normal, tangential parts normal, all with sigma^2 = k_B T / m_a
+    s_a = np.sqrt(kT_a / d["m_a"])
+    vr = np.sum(v_a * nhat, axis=1)
+    assert vr.max() <= 0.0
+    assert stats.kstest(-vr / s_a, "halfnorm").pvalue > 1e-3
+    e1 = np.cross(nhat, [0.3, -0.5, 0.8]); e1 /= np.linalg.norm(e1, axis=1)[:, None]
+    assert stats.kstest(np.sum(v_a * e1, axis=1) / s_a, "norm").pvalue > 1e-3
+    assert abs(E.mean() / kT_a - 1.5) < 4 * np.sqrt(1.5 / n)                       # <E> = 3/2 k_B T
+    assert np.allclose(E, 0.5 * d["m_a"] * np.sum(v_a ** 2, axis=1), rtol=1e-14)
+    # ion: six independent Gaussians; equipartition <m w^2 x^2> = <m v^2> = k_B T with w = q_x Omega / 2^(3/2)
+    s_v = np.sqrt(kT_i / d["m_i"])
+    w_h = abs(c.params.q[0]) * d["Omega"] / 2 ** 1.5
+    for k in range(3):
+        assert stats.kstest(v_i[:, k] / s_v, "norm").pvalue > 1e-3
+        assert stats.kstest(r_i[:, k] * w_h / s_v, "norm").pvalue > 1e-3
+    assert abs(w_h - 0.5 * d["Omega"] * np.sqrt(0.0 + c.params.q[0] ** 2 / 2)) < 1e-15 * w_h
+    assert np.abs(np.corrcoef(np.concatenate([r_i, v_i], axis=1).T) - np.eye(6)).max() < 5 / np.sqrt(n)
+    # counter-based: index and first_index commute, different cells differ
+    from dataclasses import replace as _r
+    y1, _, _ = O.generate(c.params, _r(c.launch, first_index=100), np.arange(5))
+    assert np.array_equal(y1, y0[100:105])
+    y2, _, _ = O.generate(c.params, _r(c.launch, cell=c.launch.cell + 1), np.arange(5))
+    assert not np.array_equal(y2, y0[:5])
