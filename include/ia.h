@@ -231,14 +231,15 @@ int ia_trace(ia_ctx *ctx, const double *y0_host, double phase, double h, uint32_
 int ia_get_derived(const ia_ctx *ctx, double *out16);
 
 /* Launch geometry of ia_run on this ctx (host pointers): resident warps per SM, SM count,
- * registers per thread and local-memory bytes per thread (the stack frame of the out-of-line
- * generator; ptxas reports 0 spill bytes) of persistent kernel `kernel`: 0 bulk, 1 cooperative. */
+ * registers per thread and local-memory bytes per thread (0: no stack frame, no spills) of persistent
+ * kernel `kernel`: 0 bulk (one lane per trajectory), 1 cooperative (the straggler chain's instance). */
 int ia_get_kernel_info(const ia_ctx *ctx, int kernel, int *warps_per_sm, int *n_sm, int *regs_per_thread,
                        int *local_bytes_per_thread);
 
 /* Hand-over threshold of IA_PATH_AUTO: a warp of the bulk kernel hands its running lanes over once
- * the work counter is empty and at most `lanes` of them (0..32) still run; 0 = never (the default
- * is 16: the cooperative kernel with ten trajectories per warp does the work of ~18 bulk lanes). */
+ * the work counter is empty and at most `lanes` of them (0..32) still run -- or, whatever their number,
+ * 4096 step attempts after the counter ran dry; 0 = never hand over (the default is 16: the cooperative
+ * kernel with ten trajectories per warp does the work of ~18 bulk lanes). */
 int ia_set_handoff(ia_ctx *ctx, int lanes);
 
 /* The straggler chain: the cooperative kernel is launched `levels` times in a row
