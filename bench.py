@@ -344,6 +344,8 @@ def run_ours(args):
                      "flop_per_attempted_step": FLOP_PER_STEP, "kernel": "ia_persistent_kernel<1> (bulk)",
                      "kernel_ms": bulk_ms, "steps_in_kernel": attempted - steps_coop,
                      "share_of_step_time": bulk_ms / step_avg_ms, "share_of_step_flops": 1.0 - steps_coop / max(attempted, 1),
+                     # share of the kernel's lane-steps (32 per warp and attempt) that advanced a trajectory
+                     "lane_efficiency": (attempted - steps_coop) / max(int(summ["slots_bulk"]), 1),
                      "ms_until_work_counter_empty": (int(summ["t_first_idle_ns"]) - int(summ["t_start_ns"])) * 1e-6},
         # the straggler kernel is bound by the serial latency of the longest trajectories, not by throughput
         "tail": {"kernel": f"ia_persistent_kernel<3> (cooperative, 3 lanes per trajectory), chain of {levels} launches",

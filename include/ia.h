@@ -155,7 +155,9 @@ typedef struct {
     uint64_t n_handoff;         /* trajectories finished by the cooperative kernel after a hand-over */
     uint64_t steps_coop;        /* attempted steps (incl. localisation) they took there              */
     uint64_t t_bulk_end_ns;     /* last %globaltimer over the warps of the bulk kernel               */
-    uint64_t reserved[13];
+    uint64_t slots_bulk;        /* 32 x (step attempts of every warp of the bulk kernel): attempted steps there /
+                                   slots_bulk = the share of lane-steps that advanced a trajectory            */
+    uint64_t reserved[12];
     /* Lifetimes of the complexes (n_coll >= 2), quarter-octave bins of q = t_life / T_rf (PAPER.md:34,40,
      * Fig. 2: the fraction of complexes still alive after t is 1 - cumulative sum / n_complex; R17):
      * bin b = clamp(ilogb(((q q) (q q))) + 8, 0, 63), products rounded separately, i.e. bin b holds

@@ -253,15 +253,24 @@ int run_one(const Derived &D, const double y0[12], double phase, oracle_outcome 
             /* exit, reading R7: first upward crossing of |d| = r0 */
             if (r2_new > r0sq && s_new > 0.0) {
                 /* localise: Newton on g(hk) = |d(t_n + hk)|^2 - r0^2 over uncontrolled steps from
-                 * (t_n, y_n), until |g| <= 1e-13 r0^2, at most 8 iterations */
-                double hk = h, g = r2_new - r0sq, gp = 2.0 * s_new;
+                 * (t_n, y_n), until |g| <= 1e-13 r0^2.  Reading R7 as amended: the iterate is kept inside the
+                 * bracket [lo, hi] (g(hi) > 0 known, lo = 0 where the trajectory was still inside): a Newton
+                 * proposal that leaves it -- a near-tangential exit, d.w ~ 0 -- is replaced by the midpoint;
+                 * otherwise one uncontrolled step of many rf periods can blow the ion's state up.  At most
+                 * 60 iterations (a bracket of 2^-60 h). */
+                double hk = h, g = r2_new - r0sq;
+                double lo = 0.0, hi = h;
                 uint32_t nloc = 0;
-                while (std::fabs(g) > 1e-13 * r0sq && nloc < 8) {
-                    hk = hk - g / gp;
+                while (std::fabs(g) > 1e-13 * r0sq && nloc < 60) {
+                    if (nloc > 0) {
+                        if (g > 0.0) hi = hk; else lo = hk;
+                    }
+                    double hn = hk - g / (2.0 * s_new);
+                    if (!(s_new > 0.0 && hn > lo && hn < hi)) hn = 0.5 * (lo + hi);
+                    hk = hn;
                     dp5_step(D, tf, phase, y, k1, hk, ynew, k7, e);
                     sep(ynew, &r2_new, &s_new);
                     g = r2_new - r0sq;
-                    gp = 2.0 * s_new;
                     ++nloc;
                 }
                 out->n_loc = nloc;

@@ -83,7 +83,7 @@ SUMMARY_DTYPE = np.dtype([("n_done", "<u8"), ("n_status", "<u8", (5,)), ("n_comp
                           ("sum_ke", "<f8"), ("sum_ke2", "<f8"), ("hist_ncoll", "<u8", (IA_HIST_BINS,)),
                           ("t_first_idle_ns", "<u8"), ("t_start_ns", "<u8"), ("t_end_ns", "<u8"),
                           ("warn", "<u8"), ("n_handoff", "<u8"), ("steps_coop", "<u8"), ("t_bulk_end_ns", "<u8"),
-                          ("reserved", "<u8", (13,)), ("hist_tlife", "<u8", (IA_LIFE_BINS,))])
+                          ("slots_bulk", "<u8"), ("reserved", "<u8", (12,)), ("hist_tlife", "<u8", (IA_LIFE_BINS,))])
 RECORD_BYTES, SUMMARY_BYTES, IC_DUMP_COLS = 64, 1024, 14
 assert RECORD_DTYPE.itemsize == RECORD_BYTES and SUMMARY_DTYPE.itemsize == SUMMARY_BYTES
 

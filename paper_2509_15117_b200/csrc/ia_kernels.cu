@@ -196,7 +196,8 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
         ia_record *rec[IA_THREADS];   /* outputs of the run the group's trajectory belongs to */
         ia_summary *sum[IA_THREADS];
         unsigned steps_in[IA_THREADS], n_coll[IA_THREADS], n_tp[IA_THREADS], n_loc[IA_THREADS], steps_rej[IA_THREADS],
-            cnt[IA_THREADS], wexh[IA_THREADS];
+            cnt[IA_THREADS], wexh[IA_THREADS], iters[IA_THREADS];
+        double loc_lo[IA_THREADS], loc_hi[IA_THREADS]; /* bracket of the exit localisation (R7) */
     } sh;
     double &t_first = sh.t_first[threadIdx.x], &t_last = sh.t_last[threadIdx.x], &phase = sh.phase[threadIdx.x],
            &s_old = sh.s_old[threadIdx.x];
@@ -209,6 +210,8 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
              &n_loc = sh.n_loc[threadIdx.x], &steps_rej = sh.steps_rej[threadIdx.x];
     unsigned &cnt = sh.cnt[threadIdx.x]; /* warp-uniform: step attempts since the queue ran dry */
     cnt = 0;
+    unsigned &iters = sh.iters[threadIdx.x]; /* warp-uniform: step attempts of this warp so far */
+    iters = 0;
     t_first = 0.0; t_last = 0.0; slot = 0; steps_in = 0; n_coll = 0; n_tp = 0; n_loc = 0; steps_rej = 0;
     int mode = MODE_IDLE;
     bool failed = false;
@@ -445,13 +448,13 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
                 ++n_coll;
             }
         }
-        /* exit (R7): first upward crossing of |d| = r0, localised by Newton on
+        /* exit (R7): first upward crossing of |d| = r0, localised by bracketed Newton on
          * g(hk) = |d(t_n + hk)|^2 - r0^2 over uncontrolled steps from (t_n, y_n) */
         const bool exitc = acc && (so.r2n > P.r0sq) && (so.s_new > 0.0);
         bool loc_done = false;
         if (loc) {
             ++n_loc;
-            loc_done = g_small || n_loc >= 8u;
+            loc_done = g_small || n_loc >= 60u;
         }
         fin_exit = (exitc && g_small) || loc_done;
         const bool newton = (exitc && !g_small) || (loc && !loc_done);
@@ -482,8 +485,23 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
             failed = commit ? false : (rej ? true : failed);
         }
         if (newton) {
-            h = hs - g * ia_rcp(2.0 * so.s_new);
-            if (exitc) n_loc = 0u;
+            /* Newton on g kept inside the bracket [lo, hi] of step sizes from (t_n, y_n): g(hi) > 0 is known,
+             * lo = 0 where the trajectory was still inside.  A proposal that leaves the bracket (near-tangential
+             * exit, d.w ~ 0) is replaced by the midpoint -- one uncontrolled step of many rf periods would blow
+             * the ion's state up.  NaN compares false and ends in the midpoint too. */
+            double lo = 0.0, hi = hs;
+            if (exitc) {
+                n_loc = 0u;
+            } else {
+                lo = sh.loc_lo[threadIdx.x];
+                hi = sh.loc_hi[threadIdx.x];
+                if (g > 0.0) hi = hs; else lo = hs;
+            }
+            double hn = hs - g * ia_rcp(2.0 * so.s_new);
+            if (!(so.s_new > 0.0 && hn > lo && hn < hi)) hn = 0.5 * (lo + hi);
+            h = hn;
+            sh.loc_lo[threadIdx.x] = lo;
+            sh.loc_hi[threadIdx.x] = hi;
             mode = MODE_LOC;
         }
         fin = -1;
@@ -503,6 +521,7 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
         ++it;
         } while (!__any_sync(IA_FULL, fin >= 0) && it < IA_INNER);
         cnt += it;
+        iters += it;
 
         if (__any_sync(IA_FULL, fin >= 0)) {
             /* observables (R10) + record (a10) + ensemble reduction (a11); the velocity vectors of the
@@ -569,6 +588,8 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
         const unsigned long long t1 = ia_globaltimer();
         atomicMax((unsigned long long *)&O.summary->t_end_ns, t1);
         if (!resume) atomicMax((unsigned long long *)&O.summary->t_bulk_end_ns, t1);
+        if (!resume && LPT == 1)
+            atomicAdd((unsigned long long *)&O.summary->slots_bulk, (unsigned long long)iters * PER_WARP);
     }
 }
 

@@ -2,7 +2,9 @@
 cell: ensemble results (complex-formation probability, mean ion energy gain, collision-count histogram, survival) and
 device times of the two kernels from the library's own CUDA events.
 
-    python -m paper_2509_15117_b200.sweep --configs 0,2,3,4 [--scale 1.0] [--thermal]
+    python -m paper_2509_15117_b200.sweep --configs 0,2,3:0:10,4,thermal [--scale 1.0]
+
+A config may carry a slice of its cells (3:0:10 = cells 0..9 of config 3: the D_e = 0.1 K and 1 K rows).
 
 --scale shrinks every cell (trajectories per cell = max(1024, scale * the config's own size)).  Marshalling and
 printing only: every number comes out of ia_run's summary.
@@ -66,8 +68,11 @@ def main():
         raise SystemExit("sweep needs a CUDA device: the propagator has no CPU fallback")
     torch.cuda.set_device(args.device)
     peak = P.ia_fp64_peak(args.device, 300.0)["tflops"]
-    for which in args.configs.split(","):
-        for cell in cells_of(which.strip(), args.scale):
+    for item in args.configs.split(","):
+        which, _, sl = item.strip().partition(":")
+        lo, _, hi = sl.partition(":")
+        cells = cells_of(which, args.scale)
+        for cell in cells[int(lo or 0):int(hi) if hi else len(cells)]:
             n = cell.launch.n
             with P.Context(cell.params, device=args.device) as ctx:
                 rec, summ, _ = ctx.alloc(n)
@@ -88,6 +93,7 @@ def main():
                 "rk_steps": steps, "steps_per_trajectory": steps / n,
                 "bulk_ms": t["bulk_ms"], "chain_ms": t["coop_ms"],
                 "bulk_frac_of_dfma_peak": FLOP_PER_STEP * (steps - int(s["steps_coop"])) / (t["bulk_ms"] * 1e-3) / 1e12 / peak,
+                "bulk_lane_efficiency": (steps - int(s["steps_coop"])) / max(int(s["slots_bulk"]), 1),
                 "p_complex": int(s["n_complex"]) / n, "n_status": [int(x) for x in s["n_status"]],
                 "mean_ke_ion_uK": (float(s["sum_ke"]) / max(n_esc, 1)) / KB_EH_PER_K * 1e6,
                 "hist_ncoll": [int(x) for x in s["hist_ncoll"][:12]],

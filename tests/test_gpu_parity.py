@@ -414,9 +414,14 @@ def test_config1_full_grid_in_the_bench_configuration(P):
     assert int(summ["steps_acc"]) == int(rec["steps_acc"].astype(np.int64).sum())
     assert np.array_equal(summ["hist_tlife"], O.life_bins(rec["t_life"], rec["n_coll"], O.derive(cell.params)["T_rf"]))
     assert int(summ["n_handoff"]) > 0 and int(summ["steps_coop"]) > 0
+    # lane efficiency of the bulk kernel: attempted steps there over 32 x (attempts of its warps)
+    in_bulk = int(summ["steps_acc"]) + int(summ["steps_rej"]) + int(summ["steps_loc"]) - int(summ["steps_coop"])
+    assert 0.85 < in_bulk / int(summ["slots_bulk"]) <= 1.0
     esc = rec["status"] == 0
     assert abs(summ["sum_ke"] - rec["ke_ion"][esc].sum()) <= 1e-10 * rec["ke_ion"][esc].sum()
     assert np.all(rec["status"] <= 1) and (rec["status"] == 1).sum() < 100     # a few complexes outlive t_max
+    # every exit localisation converged inside its bracket (R7): no blown-up ion state among the escaped
+    assert rec["n_loc"].max() < 60 and rec["ke_ion"][esc].max() < 1e4 * 1e-6 * 3.1668115634564e-6
     assert np.all(rec["n_coll"][rec["status"] == 0] >= 1)                      # head-on: every escape bounced once
 
 
@@ -481,3 +486,22 @@ def test_thermal_run_ensemble(P):
     assert int(summ["n_done"]) == cell.launch.n
     assert int(summ["n_complex"]) == int((rec["n_coll"] >= 2).sum())
     assert np.array_equal(summ["hist_ncoll"], S.ncoll_bins(rec["n_coll"]).astype(np.uint64))
+
+
+def test_exit_localisation_is_safeguarded_on_a_million_chaotic_trajectories(P):
+    """Regression for reading R7 as amended: config 2's Cs 3 uK cell (2^20 trajectories, t_max cut to 300 T_rf).
+    With plain Newton one near-tangential exit in a million took an uncontrolled step of many rf periods and left
+    with an ion energy of 1e21 uK, which alone set the ensemble mean.  With the bracket every localisation
+    converges and the largest energy of an escaped ion stays at the scale of the well depth."""
+    cell = I.config2()[21]
+    assert cell.name.startswith("config2_Cs133_3uK")
+    cell = replace(cell, params=replace(cell.params, t_max_rf=300.0))
+    with P.Context(cell.params) as ctx:
+        rec, summ, _ = ctx.run_sync(cell.launch)
+    esc = rec["status"] == 0
+    kB = 3.1668115634564e-6
+    ke_uK = rec["ke_ion"][esc] / kB * 1e6
+    print(f"\nCs 3 uK: escaped {esc.sum()}, max ke_ion {ke_uK.max():.4g} uK, mean {ke_uK.mean():.4g} uK, max n_loc {rec['n_loc'].max()}")
+    assert rec["n_loc"].max() < 60
+    assert ke_uK.max() < 1e5 and 5.0 < ke_uK.mean() < 100.0
+    assert abs(float(summ["sum_ke"]) - rec["ke_ion"][esc].sum()) <= 1e-10 * rec["ke_ion"][esc].sum()
