@@ -72,36 +72,59 @@ def main():
         which, _, sl = item.strip().partition(":")
         lo, _, hi = sl.partition(":")
         cells = cells_of(which, args.scale)
-        for cell in cells[int(lo or 0):int(hi) if hi else len(cells)]:
-            n = cell.launch.n
-            with P.Context(cell.params, device=args.device) as ctx:
-                rec, summ, _ = ctx.alloc(n)
+        cells = cells[int(lo or 0):int(hi) if hi else len(cells)]
+        # consecutive cells of one (species, trap, D_e, tolerances) cell -- config 4's batches of one Philox stream --
+        # share a ctx and run as one generation: bulk kernels back to back, one straggler chain for all of them
+        groups = []
+        for cell in cells:
+            if groups and groups[-1][0].params == cell.params and len(groups[-1]) < 64:
+                groups[-1].append(cell)
+            else:
+                groups.append([cell])
+        for group in groups:
+            with P.Context(group[0].params, device=args.device) as ctx:
+                ctx.set_pipeline(len(group) if len(group) > 1 else 0)
+                bufs = [ctx.alloc(c.launch.n) for c in group]
                 ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 ev0.record()
-                ctx.run(cell.launch, records=rec, summary=summ)
+                for c, (rec, summ, _) in zip(group, bufs):
+                    ctx.run(c.launch, records=rec, summary=summ)
+                ctx.join()
                 ev1.record()
                 torch.cuda.synchronize()
-                t = ctx.timing(0)
+                times = [ctx.timing(len(group) - 1 - k) for k in range(len(group))]
                 T_rf = ctx.derived["T_rf"]
-            s = P.view_summary(summ)
             wall = ev0.elapsed_time(ev1) * 1e-3
-            steps = int(s["steps_acc"]) + int(s["steps_rej"]) + int(s["steps_loc"])
-            n_esc = int(s["n_status"][0])
-            tt, S = Ob.survival_curve(s, T_rf)
-            line = {
-                "cell": cell.name, "n": n, "seconds": wall, "trajectories_per_s": n / wall, "rk_steps_per_s": steps / wall,
-                "rk_steps": steps, "steps_per_trajectory": steps / n,
-                "bulk_ms": t["bulk_ms"], "chain_ms": t["coop_ms"],
-                "bulk_frac_of_dfma_peak": FLOP_PER_STEP * (steps - int(s["steps_coop"])) / (t["bulk_ms"] * 1e-3) / 1e12 / peak,
-                "bulk_lane_efficiency": (steps - int(s["steps_coop"])) / max(int(s["slots_bulk"]), 1),
-                "p_complex": int(s["n_complex"]) / n, "n_status": [int(x) for x in s["n_status"]],
-                "mean_ke_ion_uK": (float(s["sum_ke"]) / max(n_esc, 1)) / KB_EH_PER_K * 1e6,
-                "hist_ncoll": [int(x) for x in s["hist_ncoll"][:12]],
-                "survival_at_rf_periods": {f"{2.0 ** k:g}": float(S[4 * k + 7]) for k in (2, 4, 6, 8, 10)},
-                "survival_slope_beyond_40_rf": Ob.power_law_exponent(tt, S, 40.0 * T_rf),
-                "n_handoff": int(s["n_handoff"]), "warn": int(s["warn"]),
-            }
-            print(json.dumps(line), flush=True)
+            n_all = steps_all = 0
+            for cell, (rec, summ, _), t in zip(group, bufs, times):
+                n = cell.launch.n
+                s = P.view_summary(summ)
+                steps = int(s["steps_acc"]) + int(s["steps_rej"]) + int(s["steps_loc"])
+                n_all += n
+                steps_all += steps
+                n_esc = int(s["n_status"][0])
+                tt, S = Ob.survival_curve(s, T_rf)
+                own = wall if len(group) == 1 else float("nan")   # a generation shares its wall time
+                line = {
+                    "cell": cell.name, "n": n, "seconds": own, "trajectories_per_s": n / own, "rk_steps_per_s": steps / own,
+                    "rk_steps": steps, "steps_per_trajectory": steps / n,
+                    "bulk_ms": t["bulk_ms"], "chain_ms": t["coop_ms"],
+                    "bulk_frac_of_dfma_peak": FLOP_PER_STEP * (steps - int(s["steps_coop"])) / (t["bulk_ms"] * 1e-3) / 1e12 / peak,
+                    "bulk_lane_efficiency": (steps - int(s["steps_coop"])) / max(int(s["slots_bulk"]), 1),
+                    "p_complex": int(s["n_complex"]) / n, "n_status": [int(x) for x in s["n_status"]],
+                    "mean_ke_ion_uK": (float(s["sum_ke"]) / max(n_esc, 1)) / KB_EH_PER_K * 1e6,
+                    "hist_ncoll": [int(x) for x in s["hist_ncoll"][:12]],
+                    "survival_at_rf_periods": {f"{2.0 ** k:g}": float(S[4 * k + 7]) for k in (2, 4, 6, 8, 10)},
+                    "survival_slope_beyond_40_rf": Ob.power_law_exponent(tt, S, 40.0 * T_rf),
+                    "n_handoff": int(s["n_handoff"]), "warn": int(s["warn"]),
+                }
+                print(json.dumps(line), flush=True)
+            if len(group) > 1:
+                print(json.dumps({"generation": f"{group[0].name} .. {group[-1].name}", "cells": len(group), "n": n_all,
+                                  "seconds": wall, "trajectories_per_s": n_all / wall, "rk_steps": steps_all,
+                                  "rk_steps_per_s": steps_all / wall, "chain_ms": times[0]["coop_ms"],
+                                  "bulk_ms_total": sum(t["bulk_ms"] for t in times)}), flush=True)
+            del bufs
 
 
 if __name__ == "__main__":

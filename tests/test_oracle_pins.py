@@ -563,3 +563,26 @@ def test_thermal_generator_distributions():
     assert np.array_equal(y1, y0[100:105])
     y2, _, _ = O.generate(c.params, _r(c.launch, cell=c.launch.cell + 1), np.arange(5))
     assert not np.array_equal(y2, y0[:5])
+
+
+def test_exit_localisation_lands_on_the_sphere_inside_the_detecting_step():
+    """Reading R7 (amended): for trajectories that were inside the r0 sphere, the recorded exit lies on the sphere to
+    1e-13 r0^2 in |d|^2, later than the last accepted state, after fewer than 60 localisation steps -- on a stress
+    ensemble with a hot, far-swinging ion and loose tolerances (large steps, oblique crossings of |d| = r0)."""
+    from dataclasses import replace as _r
+    c = I.thermal("Li7", 100.0, n=400)
+    p = _r(c.params, rtol=1e-5, atol=1e-7, t_max_rf=200.0)
+    L = _r(c.launch, T_ion_uK=300.0)
+    y0, ph, _ = O.generate(p, L, np.arange(400))
+    checked = 0
+    for k in range(400):
+        out, path = O.run(p, y0[k], ph[k], path_cap=100000)
+        if out["status"] != 0:
+            continue
+        dd = np.linalg.norm(path[:, 4:7] - path[:, 1:4], axis=1)
+        if not (dd[:-1] < p.r0_a0).any():
+            continue                      # started outside and never came in: the exit is the first outward step
+        checked += 1
+        assert abs(dd[-1] ** 2 - p.r0_a0 ** 2) <= 2e-13 * p.r0_a0 ** 2
+        assert path[-2, 0] < out["t_dwell"] and out["n_loc"] < 60
+    assert checked > 100
