@@ -261,7 +261,9 @@ int run_one(const Derived &D, const double y0[12], double phase, oracle_outcome 
                 double hk = h, g = r2_new - r0sq;
                 double lo = 0.0, hi = h;
                 uint32_t nloc = 0;
-                while (std::fabs(g) > 1e-13 * r0sq && nloc < 60) {
+                /* a trajectory that was already outside at t_n (a thermal start beyond r0 that never came in)
+                 * has no crossing to localise: it ends with the detecting step */
+                while (r2_old < r0sq && std::fabs(g) > 1e-13 * r0sq && nloc < 60) {
                     if (nloc > 0) {
                         if (g > 0.0) hi = hk; else lo = hk;
                     }

@@ -198,6 +198,7 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
         unsigned steps_in[IA_THREADS], n_coll[IA_THREADS], n_tp[IA_THREADS], n_loc[IA_THREADS], steps_rej[IA_THREADS],
             cnt[IA_THREADS], wexh[IA_THREADS], iters[IA_THREADS];
         double loc_lo[IA_THREADS], loc_hi[IA_THREADS]; /* bracket of the exit localisation (R7) */
+        double r2_cur[IA_THREADS];                     /* |d|^2 at the current (last committed) state */
     } sh;
     double &t_first = sh.t_first[threadIdx.x], &t_last = sh.t_last[threadIdx.x], &phase = sh.phase[threadIdx.x],
            &s_old = sh.s_old[threadIdx.x];
@@ -269,6 +270,7 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
                         Y.Ai[a] = H->A1[ax]; Y.Aa[a] = H->A1[3 + ax];
                     }
                     tf = H->tf; h = H->h; phase = H->phase; s_old = H->s_old;
+                    sh.r2_cur[threadIdx.x] = H->r2_cur;
                     t_first = H->t_first; t_last = H->t_last; slot = H->slot;
                     out_rec = H->records; out_sum = H->summary;
                     n_per = H->n_per; n_coll = H->n_coll; n_tp = H->n_tp;
@@ -339,6 +341,7 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
                         if (h < P.h_min) h = P.h_min;
                         const double W[3] = {ic.v[3] - ic.v[0], ic.v[4] - ic.v[1], ic.v[5] - ic.v[2]};
                         s_old = ia_dot3<true>(D, W);
+                        sh.r2_cur[threadIdx.x] = r2;
 #pragma unroll
                         for (int a = 0; a < NA; ++a) {
                             const unsigned ax = L.axis0 + a;
@@ -387,6 +390,7 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
                     }
                     if (L.leader) {
                         H->tf = tf; H->h = h; H->phase = phase; H->s_old = s_old;
+                        H->r2_cur = sh.r2_cur[threadIdx.x];
                         H->t_first = t_first; H->t_last = t_last; H->slot = slot;
                         H->records = out_rec; H->summary = out_sum;
                         H->n_per = n_per; H->n_coll = n_coll; H->n_tp = n_tp;
@@ -451,13 +455,17 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
         /* exit (R7): first upward crossing of |d| = r0, localised by bracketed Newton on
          * g(hk) = |d(t_n + hk)|^2 - r0^2 over uncontrolled steps from (t_n, y_n) */
         const bool exitc = acc && (so.r2n > P.r0sq) && (so.s_new > 0.0);
+        /* a trajectory that was already outside at t_n (a thermal start beyond r0 that never came in) has no
+         * crossing to localise: it ends with the detecting step */
+        bool no_root = false;
+        if (exitc) no_root = sh.r2_cur[threadIdx.x] >= P.r0sq;
         bool loc_done = false;
         if (loc) {
             ++n_loc;
             loc_done = g_small || n_loc >= 60u;
         }
-        fin_exit = (exitc && g_small) || loc_done;
-        const bool newton = (exitc && !g_small) || (loc && !loc_done);
+        fin_exit = (exitc && (g_small || no_root)) || loc_done;
+        const bool newton = (exitc && !g_small && !no_root) || (loc && !loc_done);
         const bool commit = acc && !exitc;
         const bool underflow = rej && (hs <= P.h_min);
         /* commit the accepted step: y <- ynew, k1 <- k7 (FSAL), t <- t + h with the time kept folded (R9) */
@@ -475,7 +483,10 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
                 Y.Ai[a] = commit ? N.Ai[a] : Y.Ai[a];
                 Y.Aa[a] = commit ? N.Aa[a] : Y.Aa[a];
             }
-            if (commit) s_old = so.s_new;
+            if (commit) {
+                s_old = so.s_new;
+                sh.r2_cur[threadIdx.x] = so.r2n;
+            }
         }
         /* step size of the next attempt (R5) */
         {

@@ -38,7 +38,7 @@ struct IaHand {
     ia_summary *summary; /* kernel can finish the hand-overs of several runs (ia_set_pipeline)                */
     unsigned steps_in;   /* attempted steps before the first hand-over */
     unsigned pad32;
-    unsigned long long pad;
+    double r2_cur;       /* |d|^2 at the current state (decides whether an exit can be localised, R7) */
 };
 static_assert(sizeof(IaHand) == 256, "IaHand is 256 bytes");
 
