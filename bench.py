@@ -338,8 +338,8 @@ def run_ours(args):
         "roofline": {"bound": "alu", "achieved": achieved_tflops, "peak": peak["tflops"], "unit": "TFLOP/s",
                      "frac": achieved_tflops / peak["tflops"],
                      # dram__bytes_read.sum + dram__bytes_write.sum of one K1 launch on this workload from the ncu --set full
-                     # capture in profiles/r01d_final_round1.md (the 16.8 MB of records are still in L2 when the kernel ends)
-                     "traffic": 110592 if cell.name.startswith("config1_") and args.n_side == 512 and args.t_max_rf == 0.0 else None,
+                     # capture in profiles/r01e_end_of_round.md (the 16.8 MB of records are still in L2 when the kernel ends)
+                     "traffic": 111104 if cell.name.startswith("config1_") and args.n_side == 512 and args.t_max_rf == 0.0 else None,
                      "peak_source": "ia_fp64_peak (DFMA chains on all SMs, measured in this run); nominal 37.2",
                      "flop_per_attempted_step": FLOP_PER_STEP, "kernel": "ia_persistent_kernel<1> (bulk)",
                      "kernel_ms": bulk_ms, "steps_in_kernel": attempted - steps_coop,

@@ -2,21 +2,26 @@
  * ia_kernels.cu -- the persistent propagation kernels (K1 bulk, K5 straggler), the initial-condition
  * generator (K2) and the verification kernels (K3).  Compiled with -fmad=false: see ia_dev.cuh.
  *
- * ia_persistent_kernel<LPT>: state, accelerations of all seven stages, step size and event
- * bookkeeping live in registers; nothing per step touches memory.  A group of LPT lanes owns one
- * trajectory.  A group whose trajectory has terminated writes its 64-byte record, adds to the
- * ensemble summary and takes the next index from a global work counter (one atomicAdd per
- * warp-refill), so warps stay full although trajectory lengths span 10^3..10^7 steps
- * (DESIGN.md "Persistent loop").  Exit localisation (reading R7) re-uses the same
- * step body with the group in mode LOC, so the warp never diverges on it.
+ * ia_persistent_kernel<LPT, RESUME>: state, accelerations of all seven stages and step size live in
+ * registers, what is touched only when a trajectory starts, bounces or ends in one shared-memory struct;
+ * nothing per step touches global memory.  A group of LPT lanes owns one trajectory.  A group whose
+ * trajectory has terminated writes its 64-byte record, adds to the ensemble summary and takes the next
+ * index from a global work counter (one atomicAdd per warp-refill), so warps stay full although
+ * trajectory lengths span 10^3..10^7 steps.  Exit localisation
+ * (reading R7) re-uses the same step body with the group in mode LOC, so the warp never diverges on it.
+ * The step loop proper is an inner loop of up to IA_INNER attempts that is left when a trajectory of the
+ * warp terminates; counter, queue and budget logic sit outside it and out of its registers.
  *
- *   K1 = <1>: one lane per trajectory, the throughput layout.  Once the work counter is empty and a
- *        warp is down to `handoff_lanes` running lanes it writes their states to a queue and exits.
- *   K5 = <3>: three lanes per trajectory (x/y/z split), launched behind K1 on the same stream; it
- *        resumes the queued stragglers.  A third of the FP64 instructions per lane and step: what
- *        counts for the last, longest trajectories is the latency of one step, not throughput.
- * Both run the same arithmetic (ia_dev.cuh) and give bit-identical trajectories, so where a
- * trajectory is handed over does not show in its result.
+ *   K1 = <1, false>: one lane per trajectory, the throughput layout; generates its trajectories.  Once the
+ *        work counter is empty and a warp is down to `handoff_lanes` running lanes (or `budget` attempts
+ *        later at the latest) it writes their states to a queue and exits.
+ *   K5 = <3, true>: three lanes per trajectory (x/y/z split); resumes trajectories from a queue.  A third
+ *        of the FP64 instructions per lane and step: what counts for the longest trajectories is the
+ *        latency of one step.  Launched as a chain of levels (ia_api.cu): each level passes what still runs
+ *        after its budget to the next, which deals it out ten to a warp again.
+ *   <3, false>: the cooperative layout from the first step (IA_PATH_COOP_ONLY, verification).
+ * All run the same arithmetic (ia_dev.cuh) and give bit-identical trajectories, so where a trajectory is
+ * handed over does not show in its result.
  */
 #include "ia_kernels.cuh"
 

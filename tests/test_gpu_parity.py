@@ -505,3 +505,56 @@ def test_exit_localisation_is_safeguarded_on_a_million_chaotic_trajectories(P):
     assert rec["n_loc"].max() < 60
     assert ke_uK.max() < 1e5 and 5.0 < ke_uK.mean() < 100.0
     assert abs(float(summ["sum_ke"]) - rec["ke_ion"][esc].sum()) <= 1e-10 * rec["ke_ion"][esc].sum()
+
+
+# ---------------------------------------------------------------------------------------------
+# edge cases: empty and ragged launches, every termination status
+# ---------------------------------------------------------------------------------------------
+def test_edge_cases_and_termination_statuses(P):
+    import torch
+    cell = I.config0()
+    y0, ph, _ = O.generate(cell.params, cell.launch, np.arange(33))
+
+    def both(params, y, p):
+        with P.Context(params) as ctx:
+            rec, summ, _ = ctx.run_sync(I.Launch(mode=I.MODE_EXPLICIT, n=len(y)), y0=y, phase=p)
+        return rec, summ, O.run_explicit(params, y, p, nthreads=4)
+
+    # empty launch: nothing is enqueued, nothing is written
+    with P.Context(cell.params) as ctx:
+        rec_d, summ_d, _ = ctx.alloc(4)
+        rec_d.fill_(0xAB)
+        ctx.run(I.Launch(mode=I.MODE_EXPLICIT, n=0), records=rec_d, summary=summ_d)
+        ctx.run(replace(cell.launch, n=0), records=rec_d, summary=summ_d)
+        torch.cuda.synchronize()
+        assert int(P.view_summary(summ_d)["n_done"]) == 0 and bool((rec_d == 0xAB).all())
+    # one trajectory, and a ragged 33 (one warp and one lane; four cooperative warps with a partial last one)
+    for n in (1, 33):
+        rec, summ, ref = both(cell.params, y0[:n], ph[:n])
+        assert int(summ["n_done"]) == n and np.array_equal(rec["status"], ref["status"].astype(np.uint8))
+        assert np.array_equal(rec["n_coll"], ref["n_coll"]) and np.array_equal(rec["steps_acc"], ref["steps_acc"])
+        assert np.max(np.abs(rec["t_dwell"] - ref["t_dwell"]) / ref["t_dwell"]) < 1e-8
+    # status 1: the time limit falls in the free flight; the last step lands on t_max exactly
+    p1 = replace(cell.params, t_max_rf=1.5)
+    rec, summ, ref = both(p1, y0, ph)
+    assert np.all(rec["status"] == 1) and np.all(ref["status"] == 1) and int(summ["n_status"][1]) == 33
+    assert np.array_equal(rec["t_dwell"], ref["t_dwell"]) and np.array_equal(rec["steps_acc"], ref["steps_acc"])
+    assert np.max(np.abs(rec["va_f"] - ref["va_f"]) / np.abs(ref["va_f"]).max()) < 1e-12
+    # status 4: the cap on attempted steps
+    p4 = replace(cell.params, max_steps=100)
+    rec, summ, ref = both(p4, y0, ph)
+    assert np.all(rec["status"] == 4) and np.all(ref["status"] == 4)
+    assert np.all(rec["steps_acc"].astype(np.int64) + rec["steps_rej"] == 100)
+    assert np.array_equal(rec["steps_acc"], ref["steps_acc"])
+    # status 3: a non-finite initial state is recorded as such and leaves its neighbours alone
+    yb = y0.copy(); yb[5, 4] = np.nan; yb[17, 9] = np.inf
+    rec, summ, ref = both(cell.params, yb, ph)
+    assert rec["status"][5] == 3 and rec["status"][17] == 3 and int(summ["n_status"][3]) == 2
+    good = np.ones(33, dtype=bool); good[[5, 17]] = False
+    assert np.all(rec["status"][good] == 0) and np.array_equal(rec["steps_acc"][good], ref["steps_acc"][good])
+    assert np.array_equal(ref["status"][[5, 17]], [3, 3])
+    # status 2: atom on top of the ion -- the force is not finite, every step is rejected down to h_min
+    yz = y0[:3].copy(); yz[1, 3:6] = yz[1, 0:3]
+    rec, summ, ref = both(cell.params, yz, ph[:3])
+    assert rec["status"][1] == 2 and ref["status"][1] == 2 and rec["steps_acc"][1] == 0
+    assert rec["status"][0] == 0 and rec["status"][2] == 0

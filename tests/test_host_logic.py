@@ -151,6 +151,24 @@ def test_config_recipes_match_baseline_json():
     assert firsts == [k * 2 ** 24 for k in range(18)]                        # one Philox stream, advancing
 
 
+def test_thermal_cells_and_sweep_lists():
+    """The thermal bars: ion at 10 uK, full sphere, uniform phase, one Philox cell per bar,
+    none shared with configs 2-4; sweep.cells_of lists every config with its own sizes and --scale shrinks them."""
+    from paper_2509_15117_b200 import sweep
+    bars = [I.thermal(sp, T, De) for De in (1.0, 100.0) for sp in I.SPECIES_ORDER for T in I.THERMAL_T_UK]
+    assert len({b.launch.cell for b in bars}) == 50
+    used = {c.launch.cell for c in I.config2(8) + I.config3(8) + I.config4(64, 64)}
+    assert not used & {b.launch.cell for b in bars}
+    for b in bars:
+        L = b.launch
+        assert L.mode == I.MODE_THERMAL and L.domain == 1 and L.phase_mode == 1 and L.T_ion_uK == 10.0
+        assert b.params.q[0] != 0.0 and b.params.r0_a0 == 5000.0
+    assert [len(sweep.cells_of(k, 1.0)) for k in ("0", "2", "3", "4", "thermal")] == [1, 25, 20, 18, 50]
+    assert sum(c.launch.n for c in sweep.cells_of("4", 1.0)) == 300_000_000
+    assert {c.launch.n for c in sweep.cells_of("2", 1.0 / 1024)} == {1024}
+    assert sweep.cells_of("1", 1.0)[0].launch.n == 512 * 512
+
+
 def test_subgrid_and_shards_tile_the_index_range():
     idx = I.subgrid_indices(512, 8)
     assert len(idx) == 4096 and len(set(idx.tolist())) == 4096 and idx.max() < 512 * 512
