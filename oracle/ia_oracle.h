@@ -7,7 +7,7 @@
  *
  * Plain, slow, single-thread, first-order-form Dormand-Prince 5(4) (refs [22,23])
  * on the 12-variable system of PAPER.md:13-20 (Eq. 1-2).  See ia_oracle.cpp for the per-function
- * citations and DESIGN.md section "Readings" (R1..R16) for every point the paper leaves open.
+ * citations and DESIGN.md section "Readings" (R1..R18) for every point the paper leaves open.
  */
 #ifndef IA_ORACLE_H
 #define IA_ORACLE_H
