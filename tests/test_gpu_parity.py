@@ -558,3 +558,23 @@ def test_edge_cases_and_termination_statuses(P):
     rec, summ, ref = both(cell.params, yz, ph[:3])
     assert rec["status"][1] == 2 and ref["status"][1] == 2 and rec["steps_acc"][1] == 0
     assert rec["status"][0] == 0 and rec["status"][2] == 0
+
+
+def test_deep_well_cell_ensemble(P):
+    """Config 3's D_e = 100 K, q = 0.1 cell (r_e = 22 a0, D_e/E = 3e7: the numerically hardest corner), first 2,048
+    Philox indices, t_max cut to 300 T_rf so that the oracle finishes: ensemble statistics within the 99 % intervals;
+    on single-bounce trajectories the step sequences agree and the dwell times differ at the round-off floor
+    (D_e/E) eps sqrt(N) ~ 1e-7 of reading R15, not at 1e-8."""
+    cell = I.config3(n_per_cell=2048)[16]
+    assert cell.name == "config3_De100K_q0.1"
+    cell = replace(cell, params=replace(cell.params, t_max_rf=300.0))
+    with P.Context(cell.params) as ctx:
+        rec, summ, _ = ctx.run_sync(cell.launch)
+    ref = O.run_generated(cell.params, cell.launch, nthreads=NTHREADS)
+    ok, detail = _ensemble_checks(rec, ref, cell.name)
+    assert ok, detail
+    reg = (ref["n_coll"] == 1) & (rec["n_coll"] == 1) & (ref["status"] == 0) & (rec["status"] == 0)
+    same, e_t, e_dir, e_v, e_k = _compare_regular(rec[reg], ref[reg], "D_e = 100 K regular region")
+    assert reg.sum() > 500 and same.mean() >= 0.95
+    assert np.median(e_t[same]) <= 1e-5 and np.median(e_dir[same]) <= 1e-5
+    assert int(summ["n_done"]) == 2048 and rec["n_loc"].max() < 60
