@@ -57,6 +57,9 @@ def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--configs", default="0,2,3,4")
     ap.add_argument("--scale", type=float, default=1.0)
+    ap.add_argument("--t-max-rf", type=float, default=0.0,
+                    help="override every cell's time limit (rf periods): bounds the straggler chain; complexes still "
+                         "bound then are counted as such (status 1)")
     ap.add_argument("--device", type=int, default=0)
     args = ap.parse_args()
     import torch
@@ -73,6 +76,9 @@ def main():
         lo, _, hi = sl.partition(":")
         cells = cells_of(which, args.scale)
         cells = cells[int(lo or 0):int(hi) if hi else len(cells)]
+        if args.t_max_rf > 0.0:
+            import dataclasses
+            cells = [dataclasses.replace(c, params=dataclasses.replace(c.params, t_max_rf=args.t_max_rf)) for c in cells]
         # consecutive cells of one (species, trap, D_e, tolerances) cell -- config 4's batches of one Philox stream --
         # share a ctx and run as one generation: bulk kernels back to back, one straggler chain for all of them
         groups = []
