@@ -139,7 +139,7 @@ IA_DEV double ia_inv_fifth_root(double x) {
  * (Remez, absolute error, 60-digit arithmetic) on |r| <= 1.0001 pi/2: 3.9e-18 before and 4.4e-17 after
  * rounding the coefficients to double -- below half an ulp of 1, so the polynomial's own error is hidden
  * by the ~1e-16 rounding of the Horner chain (the Taylor series needs three more terms for that).
- * tests/test_host_logic.py re-evaluates these literals against a 50-digit cosine. */
+ * csrc/ia_cos_fit.py is the fit; tests/test_host_logic.py re-evaluates these literals against a 50-digit cosine. */
 #define IA_COS_C8 (+4.60897384029083775838e-14)
 #define IA_COS_C7 (-1.14629017962301774571e-11)
 #define IA_COS_C6 (+2.08765618439870221873e-09)
