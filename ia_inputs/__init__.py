@@ -170,13 +170,6 @@ def subgrid_indices(n_side: int, every: int) -> np.ndarray:
     return (ii[:, None] * np.uint64(n_side) + ii[None, :]).reshape(-1)
 
 
-def shard(n: int, rank: int, world: int) -> tuple:
-    """Contiguous index range [first, first+count) of rank `rank` out of `world` (no overlap, no gap)."""
-    base, rem = divmod(n, world)
-    first = rank * base + min(rank, rem)
-    return first, base + (1 if rank < rem else 0)
-
-
 # --- seeded explicit initial conditions (numbers only; no physics beyond placing the particles) ---
 
 def impact_ic(b_a0: float, r0_a0: float, v0_au: float) -> np.ndarray:

@@ -17,7 +17,9 @@
  * Parity pins (tests/test_oracle_*.py): tableau order conditions, potential minimum and depth,
  * force = -grad V, Newton's third law, z-axis harmonic period, Mathieu characteristic exponent,
  * classical deflection integral, energy / angular momentum / linear momentum conservation,
- * mirror symmetry, convergence order, Philox known-answer vectors.
+ * mirror symmetry, convergence order, Philox known-answer vectors, the word -> uniform map and the GRID / PHILOX
+ * direction, phase and energy maps, the error norm and every branch of the step-size law on a linear problem with
+ * a closed-form step, the collision times against the turning-point quadrature (tests/test_oracle_pins2.py).
  * Unpinned: none of the paper's figure values are recoverable (images absent), so the ensemble
  * statistics (P(complex), histograms) are "parity unpinned" against the paper -- only trend checks.
  */
@@ -347,7 +349,8 @@ void philox(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
     out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
-/* reading R2: 53-bit uniform in (0,1) from two words */
+/* reading R2: uniform in (0,1] from two words: (k + 1/2) 2^-53 with the 53-bit integer k = (we >> 5) 2^26 + (wo >> 6),
+ * the sum k + 1/2 rounded to double (exact below k = 2^52, ties-to-even from there on, so the largest k gives 1.0) */
 double u53(uint32_t we, uint32_t wo) {
     return ((double)(we >> 5) * 67108864.0 + (double)(wo >> 6) + 0.5) * (1.0 / 9007199254740992.0);
 }
@@ -531,6 +534,8 @@ int oracle_run(const oracle_params *p, const double y0[12], double phase, oracle
 void oracle_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
     philox(ctr, key, out);
 }
+
+double oracle_u53(uint32_t w_even, uint32_t w_odd) { return u53(w_even, w_odd); }
 
 int oracle_generate(const oracle_params *p, const oracle_gen *g, uint64_t index, double y0[12],
                     double *phase, double *E_au) {

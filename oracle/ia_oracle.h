@@ -73,6 +73,8 @@ int  oracle_run(const oracle_params *p, const double y0[12], double phase, oracl
                 double *path, uint64_t path_cap, uint64_t *path_len);
 /* Philox4x32-10 */
 void oracle_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
+/* reading R2: the uniform deviate in (0,1] made of two Philox words */
+double oracle_u53(uint32_t w_even, uint32_t w_odd);
 /* generate trajectory `index` (local index; global = first_index + index): y0[12], phase, E (E_h) */
 int  oracle_generate(const oracle_params *p, const oracle_gen *g, uint64_t index, double y0[12],
                      double *phase, double *E_au);

@@ -92,6 +92,8 @@ def lib() -> C.CDLL:
                                  C.c_uint64, C.POINTER(C.c_uint64)]
         L.oracle_philox4x32_10.argtypes = [C.POINTER(C.c_uint32), C.POINTER(C.c_uint32), C.POINTER(C.c_uint32)]
         L.oracle_philox4x32_10.restype = None
+        L.oracle_u53.argtypes = [C.c_uint32, C.c_uint32]
+        L.oracle_u53.restype = C.c_double
         L.oracle_generate.argtypes = [C.POINTER(OracleParams), C.POINTER(OracleGen), C.c_uint64, dp, dp, dp]
         L.oracle_run_generated.argtypes = [C.POINTER(OracleParams), C.POINTER(OracleGen),
                                            C.POINTER(C.c_uint64), C.c_uint64, C.c_uint64, C.c_void_p, C.c_int]
@@ -176,6 +178,10 @@ def philox4x32_10(ctr, key) -> np.ndarray:
     o = (C.c_uint32 * 4)()
     lib().oracle_philox4x32_10(c, k, o)
     return np.array(list(o), dtype=np.uint32)
+
+
+def u53(w_even: int, w_odd: int) -> float:
+    return lib().oracle_u53(int(w_even), int(w_odd))
 
 
 def generate(p, launch, indices) -> tuple:

@@ -31,7 +31,7 @@ def shard_launch(launch, rank: int, world: int):
 
 
 _SUM_FIELDS = ("n_done", "n_status", "n_complex", "steps_acc", "steps_rej", "steps_loc", "sum_ke", "sum_ke2",
-               "hist_ncoll", "hist_tlife", "slots_bulk")
+               "hist_ncoll", "hist_tlife", "slots_bulk", "n_handoff", "steps_coop")
 
 
 def summary_to_vector(summary) -> np.ndarray:

@@ -10,9 +10,3 @@ if ROOT not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (B200); run with -m gpu")
-
-
-def pytest_collection_modifyitems(config, items):
-    """GPU tests fail loudly (not skip) when selected on a box without a device; they are only
-    deselected by `-m "not gpu"`."""
-    return
