@@ -1,15 +1,21 @@
 #!/usr/bin/env python
-"""bench.py -- throughput of the batched ion+atom propagator on BASELINE.json configs[1]
-(Yb+ + 87Rb fractal angle map, 512x512 octant grid = 262,144 trajectories, E = 1.5 uK, t_max 1e4 T_rf).
+"""bench.py -- throughput of the batched ion+atom propagator on BASELINE.json configs[4], the largest
+single-GPU configuration (the paper's ">3x10^8 trajectories"): Yb+ + 87Rb, E log-uniform in
+[1,100] uK, full sphere, uniform rf phase, ONE Philox stream in batches of 2^24 trajectories.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--n-side 512]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload config4|config1|...]
 
-One "step" = one pass of the whole hot path (generator -> adaptive DP5(4) propagation -> events ->
-exit localisation -> observables -> record write -> ensemble reduction) over the whole grid.
-Prints ONE JSON line on rank 0.  `value` = trajectories/s with everything resident on the device;
-`e2e` = the same metric through ia_run_host with HOST buffers (explicit initial conditions copied in,
-records and summary copied out, inside the timed region).  `roofline` is against the FP64 FMA peak
-measured live by the library's DFMA microbenchmark (MEASURED_PEAKS.json carries no FP64 figure).
+One "step" = one batch of the stream through the whole hot path (generator -> adaptive DP5(4) propagation ->
+events -> exit localisation -> observables -> 64-byte record -> ensemble reduction); first_index advances from
+step to step.  The steps run as a pipeline (ia_set_pipeline): the bulk kernel of a step first resumes the
+trajectories the step before left unfinished, so the power-law tail of trajectory lengths lives in
+full warps while new trajectories keep arriving.  The timed region is K consecutive steps of the running stream,
+entered after W warm-up steps (the first of them alone and timed separately: `latency_one_step_alone_ms`) and left
+when the K-th bulk kernel ends; `value` = trajectories FINISHED inside it per second, device-resident.  The
+straggler chain that ends the stream afterwards is timed on its own (`tail`).  `e2e` = the same stream continued
+through ia_submit_host with page-locked HOST buffers (launch descriptor in, 1 GiB of records per step copied
+back inside the timed region).  `roofline` is against the FP64 FMA peak measured live by the library's DFMA
+microbenchmark (MEASURED_PEAKS.json carries no FP64 figure).  Prints ONE JSON line on rank 0.
 `--impl reference` times the CPU oracle (test infrastructure; the only other place that may run it).
 """
 from __future__ import annotations
@@ -21,10 +27,6 @@ import subprocess
 import sys
 import tempfile
 import time
-
-# One hardware work queue per stream: with the default of 8, the straggler streams of a deep pipeline would share
-# queues and their kernels would serialise behind one another (must be set before CUDA is initialised).
-os.environ.setdefault("CUDA_DEVICE_MAX_CONNECTIONS", "32")
 
 ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
@@ -40,7 +42,10 @@ METRIC = "trajectories/s"
 # stage sums 300, six accelerations 234, d.w 8, error sums 120, norm cross-products 22,
 # controller / time keeping 32.
 FLOP_PER_STEP = 886.0
-ORACLE_SAMPLE_EVERY = 8   # cpu_baseline: every 8th grid point in theta and phi (64x64 = 4,096 trajectories)
+ORACLE_SAMPLE_EVERY = 8   # oracle legs on a GRID workload: every 8th grid point in theta and phi (64x64 = 4,096)
+ORACLE_SAMPLE_PHILOX = 8192   # ... on a Philox stream: its first 8,192 indices (reference arm, per step)
+ORACLE_SAMPLE_BASELINE = 32768  # ... and for the one-shot cpu_baseline of our arm
+E2E_STEPS_MAX = 12        # steps of the end-to-end leg (1 GiB of page-locked host memory each on config 4)
 
 
 def parse():
@@ -50,10 +55,11 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--n-side", type=int, default=512)
-    ap.add_argument("--workload", default="config1",
-                    help="config1 (default, the bench line) | config0 | config2.<cell 0-24> | config3.<cell 0-19> | "
-                         "config4 (one batch): the other BASELINE.json configs, for profiling and inspection")
-    ap.add_argument("--n", type=int, default=0, help="trajectories per pass for the Philox workloads (default: "
+    ap.add_argument("--workload", default="config4",
+                    help="config4 (default, the bench line: one batch of 2^24 per step) | config1 | config0 | "
+                         "config2.<cell 0-24> | config3.<cell 0-19>: the other BASELINE.json configs, for profiling "
+                         "and inspection (a GRID workload repeats the same grid every step)")
+    ap.add_argument("--n", type=int, default=0, help="trajectories per step for the Philox workloads (default: "
                                                      "the config's own cell / batch size)")
     ap.add_argument("--t-max-rf", type=float, default=0.0,
                     help="override the time limit (rf periods) -- profiling runs only; the bench line uses the config's own")
@@ -61,9 +67,8 @@ def parse():
                     help="hand-over threshold of the bulk kernel in lanes (0 = bulk kernel only; default: the library's)")
     ap.add_argument("--path", type=int, default=0, help="ia_path: 0 production kernel pair, 1 bulk only, 2 cooperative only")
     ap.add_argument("--pipeline", type=int, default=64,
-                    help="ia_set_pipeline depth: passes per generation, i.e. how many passes share one straggler kernel "
-                         "(it runs on the library's stream while the next generation's bulk kernels run); "
-                         "0 = strictly one pass after another, both kernels of a pass back to back")
+                    help="ia_set_pipeline depth (steps between two forced straggler chains); 0 = every step on its "
+                         "own, bulk kernel and straggler chain back to back")
     ap.add_argument("--chain", default="", help="levels,budget of the straggler chain (ia_set_chain); default: the library's")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -149,13 +154,13 @@ class ClockSampler:
 
 # ---- the oracle legs (cpu_baseline and --impl reference) -----------------------------------------
 
-def oracle_sample(cell, n_side: int):
+def oracle_sample(cell, n_side: int, n_philox: int = ORACLE_SAMPLE_PHILOX):
     """Times the oracle, as it stands, on a bounded sample of the same workload: the decimated sub-grid
-    of a GRID launch, the first 4,096 indices of a Philox launch."""
+    of a GRID launch, the first n_philox indices of a Philox launch."""
     from oracle import ia_oracle as O
     cores = os.cpu_count() or 1
     if cell.launch.mode != I.MODE_GRID or cell.launch.n_theta != n_side:
-        idx = np.arange(min(cell.launch.n, 4096), dtype=np.uint64)
+        idx = np.arange(min(cell.launch.n, n_philox), dtype=np.uint64)
         t0 = time.perf_counter()
         out = O.run_generated(cell.params, cell.launch, indices=idx, nthreads=cores)
         dt = time.perf_counter() - t0
@@ -211,6 +216,9 @@ def run_ours(args):
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus:
+        raise SystemExit(f"bench.py --gpus {args.gpus} but WORLD_SIZE={world}: start it through torch.distributed.run "
+                         f"(a plain `python bench.py --gpus N` does that itself)")
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the propagator has no CPU fallback")
     torch.cuda.set_device(local)
@@ -219,15 +227,20 @@ def run_ours(args):
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         dist.init_process_group("nccl", device_id=dev)
     K, W = args.steps, max(args.warmup, 3)
+    Ke = 0 if args.no_e2e else min(K, E2E_STEPS_MAX)
 
-    # Workload: configs[1].  Trajectories are independent, so N GPUs run N grids of the same shape (weak
-    # scaling, no data-path collective): rank r maps the octant at rf phase 2 pi r / N.
+    # Workload.  Trajectories are independent, so N GPUs run N streams of the same shape (weak scaling, no
+    # data-path collective): rank r takes its own index range of the Philox stream (a GRID workload: the same
+    # grid at rf phase 2 pi r / N).
     cell = pick_workload(args)
-    if cell.launch.mode == I.MODE_GRID:
-        launch = dataclasses.replace(cell.launch, phase0=2.0 * np.pi * rank / world)
-    else:   # Philox workloads: rank r continues the same stream at index r * n
-        launch = dataclasses.replace(cell.launch, first_index=cell.launch.first_index + rank * cell.launch.n)
-    n = launch.n
+    n = cell.launch.n
+    stream_like = cell.launch.mode != I.MODE_GRID
+
+    def launch_of(step: int):
+        if stream_like:
+            return dataclasses.replace(cell.launch, path=args.path,
+                                       first_index=cell.launch.first_index + (rank * 4096 + step) * n)
+        return dataclasses.replace(cell.launch, path=args.path, phase0=2.0 * np.pi * rank / world)
 
     def barrier():
         if world > 1:
@@ -242,77 +255,95 @@ def run_ours(args):
     if args.chain:
         levels, budget = (int(x) for x in args.chain.split(","))
         ctx.set_chain(levels, budget)
-    depth = max(0, min(args.pipeline, 64, K))
-    ctx.set_pipeline(depth)
-    launch = dataclasses.replace(launch, path=args.path)
+    depth = max(0, min(args.pipeline, 64))
+    n_steps_all = W + K + Ke
+    if depth > 0 and n_steps_all - 1 > depth:
+        raise SystemExit(f"--warmup + --steps (+ {Ke} end-to-end steps) = {n_steps_all} exceeds the pipeline depth {depth} + 1")
     info = ctx.kernel_info
-    nbuf = min(K, 2 * max(depth, 1))             # passes in flight (two generations) never share an output buffer
-    recs_d = [torch.empty(n * P.RECORD_BYTES, dtype=torch.uint8, device=dev) for _ in range(nbuf)]
+    # every step of the device leg keeps its own record buffer until the stream is drained (a trajectory in flight
+    # writes into the buffer of the step it belongs to)
+    recs_d = [torch.empty(n * P.RECORD_BYTES, dtype=torch.uint8, device=dev) for _ in range(W + K)]
     summaries = torch.zeros((W + K, P.SUMMARY_BYTES), dtype=torch.uint8, device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    mk = lambda: torch.cuda.Event(enable_timing=True)
+    ev_a0, ev_a1, ev0, ev1 = mk(), mk(), mk(), mk()
 
-    for w in range(W):
-        ctx.run(launch, records=recs_d[w % nbuf], summary=summaries[w])
+    def view_all():
+        return summaries.cpu().numpy().view(P.SUMMARY_DTYPE).reshape(-1)
+
+    # warm-up step 0 on its own: bulk kernel + its straggler chain = the latency of one step alone
+    ctx.set_pipeline(0)
+    ev_a0.record()
+    ctx.run(launch_of(0), records=recs_d[0], summary=summaries[0])
+    ev_a1.record()
+    torch.cuda.synchronize(dev)
+    alone_ms = ev_a0.elapsed_time(ev_a1)
+    alone_t = ctx.timing(0)
+    # the stream proper: warm-up steps 1..W-1 fill the pipeline, then the timed region, no join in between
+    ctx.set_pipeline(depth)
+    for w in range(1, W):
+        ctx.run(launch_of(w), records=recs_d[w], summary=summaries[w])
         flush.fill_(w)
-    ctx.join()
     barrier()
+    done0 = int(view_all()["n_done"].sum())
     clocks = ClockSampler(local)
     clocks.start()
     ev0.record()
     for k in range(K):
-        # one step = one pass over the grid: its bulk kernel here; its stragglers are finished by the straggler
-        # kernel of its generation (depth 0: right behind the bulk kernel; depth > 0: one launch for `depth` passes,
-        # on the library's stream, while the next generation's bulk kernels run)
-        ctx.run(launch, records=recs_d[k % nbuf], summary=summaries[W + k])
+        ctx.run(launch_of(W + k), records=recs_d[W + k], summary=summaries[W + k])
         flush.fill_(k)                                             # L2 flush between timed iterations
-    ctx.join()                                                     # the stream waits for every straggler kernel
+    if depth == 0:
+        ctx.join()
     ev1.record()
     barrier()
     clk = clocks.stop()
-    total_s = D.all_reduce_max(ev0.elapsed_time(ev1) * 1e-3, dev)
-    kernel_times = []                              # the library's own CUDA events around each kernel
-    for back in range(K):
-        try:
-            kernel_times.append(ctx.timing(back))
-        except P.IaError:                          # older than the two generations the library keeps on record
-            break
-    n_coop_launches = K if depth == 0 else -(-K // depth)
-    summ = P.view_summary(summaries[W + K - 1])
-    bulk_ms = float(np.mean([t["bulk_ms"] for t in kernel_times]))
-    coop_ms = float(np.mean([t["coop_ms"] for t in kernel_times]))
-    attempted = int(summ["steps_acc"]) + int(summ["steps_rej"]) + int(summ["steps_loc"])
-    steps_coop = int(summ["steps_coop"])
-    recs = P.view_records(recs_d[(K - 1) % nbuf], n)
-    longest = int((recs["steps_acc"].astype(np.int64) + recs["steps_rej"]).max())
-    tot = D.all_reduce_summary(summ, dev)
-    attempted_all = tot["steps_acc"] + tot["steps_rej"] + tot["steps_loc"]
-    value = world * n * K / total_s
-    step_avg_ms = 1e3 * total_s / K
+    region_s = D.all_reduce_max(ev0.elapsed_time(ev1) * 1e-3, dev)
+    mid = view_all()
+    finished = int(D.all_reduce_sum(int(mid["n_done"].sum()) - done0, dev))     # trajectories finished inside the region
+    steps_region = int(mid["steps_kernel"][W:].sum())     # attempted steps the K timed bulk kernels executed (this rank)
+    slots_region = int(mid["slots_bulk"][W:].sum())
+    steps_region_all = int(D.all_reduce_sum(steps_region, dev))
 
-    # end to end through the host entry points: explicit initial conditions in pinned host memory -> device,
-    # records + summary -> pinned host memory, all inside the timed region (ia_submit_host x K, ia_wait)
+    # end to end: the same stream continued through the host entry points, page-locked host buffers: launch
+    # descriptor in, records copied back behind every bulk kernel (inside the timed region)
     e2e = None
-    if not args.no_e2e:
-        ic = ctx.generate(launch)                                   # untimed: the inputs of the e2e leg
-        y0 = torch.from_numpy(np.ascontiguousarray(ic[:, :12])).pin_memory()
-        ph = torch.from_numpy(np.ascontiguousarray(ic[:, 12])).pin_memory()
-        rec_h = [torch.empty(n * P.RECORD_BYTES, dtype=torch.uint8).pin_memory() for _ in range(nbuf)]
-        sum_h = [torch.zeros(P.SUMMARY_BYTES, dtype=torch.uint8).pin_memory() for _ in range(nbuf)]
-        lx = I.Launch(mode=I.MODE_EXPLICIT, n=n)
-        cl = P.make_launch(lx, y0, ph)
-        P.ia_run_host(ctx.handle, cl, rec_h[0], sum_h[0])           # warm-up (staging allocation)
+    if Ke > 0:
+        rec_h = [torch.empty(n * P.RECORD_BYTES, dtype=torch.uint8).pin_memory() for _ in range(Ke)]
+        sum_h = [torch.zeros(P.SUMMARY_BYTES, dtype=torch.uint8).pin_memory() for _ in range(Ke)]
+        cls = [P.make_launch(launch_of(W + K + k)) for k in range(Ke)]
         barrier()
         t0 = time.perf_counter()
-        for k in range(K):
-            P.ia_submit_host(ctx.handle, cl, rec_h[k % nbuf], sum_h[k % nbuf])
-        ctx.wait()                                                  # blocks until every copy back has landed
+        for k in range(Ke):
+            P.ia_submit_host(ctx.handle, cls[k], rec_h[k], sum_h[k])
+        ctx.sync()                                                  # every bulk kernel and every copy back has landed
         e2e_s = D.all_reduce_max(time.perf_counter() - t0, dev)
-        done = int(sum_h[(K - 1) % nbuf].numpy().view(P.SUMMARY_DTYPE)[0]["n_done"])
-        assert done == n, (done, n)
-        e2e = {"value": world * n * K / e2e_s, "unit": "trajectories/s",
-               "h2d_bytes_per_step": int(y0.numel() * 8 + ph.numel() * 8),
-               "d2h_bytes_per_step": int(rec_h[0].numel() + sum_h[0].numel()), "ms_per_step": 1e3 * e2e_s / K}
+        import ctypes
+        e2e = {"value": world * n * Ke / e2e_s, "unit": "trajectories/s", "steps": Ke,
+               "h2d_bytes_per_step": ctypes.sizeof(P.ia_launch),
+               "d2h_bytes_per_step": int(rec_h[0].numel()), "ms_per_step": 1e3 * e2e_s / Ke,
+               "note": "ia_submit_host x steps + ia_sync on the running pipeline: generator mode, so the input of a step is "
+                       "its launch descriptor; records of a step are copied to page-locked host memory behind its bulk "
+                       "kernel; trajectories still in flight then (<= one per lane) report at ia_wait"}
+    # the end of the stream: one straggler chain for what the last bulk kernel left
+    t0 = time.perf_counter()
+    ctx.wait()
+    ctx.join()
+    torch.cuda.synchronize(dev)
+    drain_s = D.all_reduce_max(time.perf_counter() - t0, dev)
+    if Ke > 0:
+        done_h = sum(int(s.numpy().view(P.SUMMARY_DTYPE)[0]["n_done"]) for s in sum_h)
+        assert done_h == Ke * n, (done_h, Ke * n)
+        st = rec_h[-1].numpy().view(P.RECORD_DTYPE)["status"]
+        assert int((st > 4).sum()) == 0
+    fin = view_all()
+    assert int(fin["n_done"].sum()) == (W + K) * n, (int(fin["n_done"].sum()), (W + K) * n)
+    chain_t = ctx.timing(0)
+    kernel_ms = [ctx.timing(Ke + K - 1 - k)["bulk_ms"] for k in range(K)]   # the K timed bulk kernels
+    bulk_ms = float(np.mean(kernel_ms))
+    tot = D.all_reduce_summary(D.sum_summaries(fin[W:]), dev)
+    attempted = tot["steps_acc"] + tot["steps_rej"] + tot["steps_loc"]
+    recs = P.view_records(recs_d[W + K - 1], n)
+    longest = int((recs["steps_acc"].astype(np.int64) + recs["steps_rej"]).max())
     ctx.close()
     if world > 1:
         dist.barrier(device_ids=[local])
@@ -321,45 +352,52 @@ def run_ours(args):
             dist.destroy_process_group()
         return
 
-    # roofline of the kernel that does the arithmetic: the bulk kernel (one lane per trajectory) over its own
-    # launch duration; the steps the straggler kernel took are not counted for it
-    achieved_tflops = FLOP_PER_STEP * (attempted - steps_coop) / (bulk_ms * 1e-3) / 1e12
+    value = finished / region_s
+    achieved_tflops = FLOP_PER_STEP * steps_region / (sum(kernel_ms) * 1e-3) / 1e12
+    whole_tflops = FLOP_PER_STEP * steps_region / region_s / 1e12
     line = {
         "metric": METRIC, "value": value, "unit": "trajectories/s", "n_gpus": world, "steps": K, "warmup": W,
-        "ms_per_step": 1e3 * total_s / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": 1e3 * region_s / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": cell.name, "trajectories_per_step_per_gpu": n, "parallelism": f"dp{world}",
+        "config": {"workload": f"{cell.name}_stream_{n}" if stream_like else cell.name,
+                   "trajectories_per_step_per_gpu": n, "parallelism": f"dp{world}",
+                   "timed_region": "K consecutive steps of a running pipeline (ia_set_pipeline): entered after W warm-up steps "
+                                   "without a join, left when the K-th bulk kernel ends; value = trajectories finished inside it; "
+                                   "the straggler chain that ends the stream is timed separately (tail)",
                    "l2": "flushed between timed iterations (256 MiB write); the kernel reads no input arrays",
                    "pipeline_depth": depth,
                    "rtol": cell.params.rtol, "atol": cell.params.atol, "t_max_rf": cell.params.t_max_rf},
-        "rk_steps_per_s": attempted_all * K / total_s,
-        "rk_steps_per_pass": attempted_all,
+        "trajectories_started_per_s": world * n * K / region_s,
+        "rk_steps_per_s": steps_region_all / region_s,
+        "rk_steps_per_step": steps_region / K,
+        "latency_one_step_alone_ms": alone_ms,
+        "one_step_alone": {"bulk_ms": alone_t["bulk_ms"], "chain_ms": alone_t["coop_ms"],
+                           "trajectories_per_s": n / (alone_ms * 1e-3)},
         "p_complex": tot["n_complex"] / max(tot["n_done"], 1), "n_status": tot["n_status"],
         "roofline": {"bound": "alu", "achieved": achieved_tflops, "peak": peak["tflops"], "unit": "TFLOP/s",
                      "frac": achieved_tflops / peak["tflops"],
-                     # dram__bytes_read.sum + dram__bytes_write.sum of one K1 launch on this workload from the ncu --set full
-                     # capture in profiles/r01e_end_of_round.md (the 16.8 MB of records are still in L2 when the kernel ends)
-                     "traffic": 111104 if cell.name.startswith("config1_") and args.n_side == 512 and args.t_max_rf == 0.0 else None,
+                     "traffic": None,
                      "peak_source": "ia_fp64_peak (DFMA chains on all SMs, measured in this run); nominal 37.2",
-                     "flop_per_attempted_step": FLOP_PER_STEP, "kernel": "ia_persistent_kernel<1> (bulk)",
-                     "kernel_ms": bulk_ms, "steps_in_kernel": attempted - steps_coop,
-                     "share_of_step_time": bulk_ms / step_avg_ms, "share_of_step_flops": 1.0 - steps_coop / max(attempted, 1),
+                     "flop_per_attempted_step": FLOP_PER_STEP, "kernel": "ia_persistent_kernel<1, IA_SRC_BOTH> (bulk)",
+                     "kernel_ms": bulk_ms, "steps_in_kernel": steps_region / K,
+                     "share_of_step_time": sum(kernel_ms) * 1e-3 / region_s,
                      # share of the kernel's lane-steps (32 per warp and attempt) that advanced a trajectory
-                     "lane_efficiency": (attempted - steps_coop) / max(int(summ["slots_bulk"]), 1),
-                     "ms_until_work_counter_empty": (int(summ["t_first_idle_ns"]) - int(summ["t_start_ns"])) * 1e-6},
-        # the straggler kernel is bound by the serial latency of the longest trajectories, not by throughput
-        "tail": {"kernel": f"ia_persistent_kernel<3> (cooperative, 3 lanes per trajectory), chain of {levels} launches",
-                 "kernel_ms": coop_ms,
-                 "launches": n_coop_launches, "passes_per_launch": K / n_coop_launches,
-                 "share_of_step_time": coop_ms * n_coop_launches / K / step_avg_ms,
-                 "trajectories_handed_over_per_pass": int(summ["n_handoff"]),
-                 "steps_in_kernel_per_pass": steps_coop, "longest_trajectory_steps": longest,
-                 "us_per_step_serial_bound": 1e3 * coop_ms / max(longest, 1),
-                 "note": "a trajectory is a serial chain: the launch cannot end before its longest one (DESIGN.md 'Tail')"},
-        "kernel_info": info, "clocks": clk, "e2e": e2e, "gpu_launches": K + n_coop_launches * levels,
+                     "lane_efficiency": steps_region / max(slots_region, 1)},
+        # every attempted step executed inside the timed region over the whole region
+        "whole_step": {"achieved": whole_tflops, "peak": peak["tflops"], "unit": "TFLOP/s",
+                       "frac": whole_tflops / peak["tflops"], "rk_steps": steps_region, "seconds": region_s},
+        # the end of the stream: a trajectory is a serial chain, so the chain lasts as long as the longest one left
+        "tail": {"kernel": f"ia_persistent_kernel<3, IA_SRC_QUEUE> (cooperative, 3 lanes per trajectory), chain of {levels} launches",
+                 "chain_ms": chain_t["coop_ms"], "drain_wall_ms": 1e3 * drain_s,
+                 "share_of_step_time": 0.0,
+                 "share_of_stream_time": chain_t["coop_ms"] * 1e-3 / (region_s + chain_t["coop_ms"] * 1e-3),
+                 "longest_trajectory_steps_last_step": longest,
+                 "note": "outside the timed region; paid once per stream, whatever its length (DESIGN.md 'Tail')"},
+        "attempted_steps_of_timed_batches": attempted,
+        "kernel_info": info, "clocks": clk, "e2e": e2e, "gpu_launches": K,
     }
     if not args.no_cpu_baseline and world == 1:
-        s = oracle_sample(cell, args.n_side)
+        s = oracle_sample(cell, args.n_side, ORACLE_SAMPLE_BASELINE)
         line["cpu_baseline"] = {"value": s["n"] / s["seconds"], "unit": "trajectories/s", "cores": s["cores"],
                                 "kind": "oracle", "sample": s["sample"], "rk_steps_per_s": s["steps"] / s["seconds"]}
     print(json.dumps(line), flush=True)
@@ -367,10 +405,23 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def spawn_ranks(args) -> int:
+    """`python bench.py --gpus N` without a launcher: start the N ranks ourselves, the way the driver does."""
+    import socket
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__), *sys.argv[1:]]
+    return subprocess.call(cmd)
+
+
 def main():
     args = parse()
     if args.impl == "reference":
         run_reference(args)
+    elif args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        sys.exit(spawn_ranks(args))
     else:
         run_ours(args)
 

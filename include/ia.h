@@ -21,7 +21,8 @@
  *   - "device" pointers are CUDA device pointers valid on the ctx's device; "host" pointers are
  *     ordinary process memory.  Each argument says which it is.
  *   - The library never allocates, frees or keeps caller memory.  A ctx owns only its own scratch
- *     (work counter, host-call staging buffers).
+ *     (work counters, hand-over queues, host-call staging buffers).  Which calls block the host or
+ *     allocate is listed at ia_submit_host below.
  *   - Every function returns IA_OK (0) or a negative ia_status; on failure nothing was launched.
  *     A failed *trajectory* is not a call error: see ia_record.status.
  *   - A ctx is not thread-safe.  Two ctxs may run concurrently on different streams.
@@ -157,7 +158,10 @@ typedef struct {
     uint64_t t_bulk_end_ns;     /* last %globaltimer over the warps of the bulk kernel               */
     uint64_t slots_bulk;        /* 32 x (step attempts of every warp of the bulk kernel): attempted steps there /
                                    slots_bulk = the share of lane-steps that advanced a trajectory            */
-    uint64_t reserved[12];
+    uint64_t steps_kernel;      /* attempted steps (incl. localisation) the bulk kernel of THIS run executed,
+                                   whichever run their trajectories belong to (ia_set_pipeline: it also advances
+                                   what earlier runs left unfinished)                                          */
+    uint64_t reserved[11];
     /* Lifetimes of the complexes (n_coll >= 2), quarter-octave bins of q = t_life / T_rf (PAPER.md:34,40,
      * Fig. 2: the fraction of complexes still alive after t is 1 - cumulative sum / n_complex; R17):
      * bin b = clamp(ilogb(((q q) (q q))) + 8, 0, 63), products rounded separately, i.e. bin b holds
@@ -184,25 +188,40 @@ int ia_run_host(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *host_out
 
 /* Pipelining of successive runs.  Trajectory lengths are power-law distributed
  * (PAPER.md:40): the last few trajectories of a launch take 10^3 times longer than the median, and a
- * trajectory is a serial chain, so the straggler kernel of a run outlasts its bulk kernel by far.
- * With depth d > 0 (at most 64) runs are grouped into generations of d: ia_run enqueues only the bulk
- * kernel, whose hand-overs go to a queue the generation shares; after the d-th run (or at ia_join) ONE
- * straggler kernel finishes the hand-overs of the whole generation, on a ctx-owned stream, so that the
- * caller's stream goes on with the bulk kernels of the next generation meanwhile (two generation
- * buffers; the third generation waits, on the device, for the first).  Each queue entry carries the
- * outputs of its own run.  depth 0 (the default) keeps both kernels of every run on the caller's stream.
- * With depth > 0 the outputs of ia_run are valid only after ia_join: it enqueues the straggler kernel of
- * an incomplete generation and makes `cuda_stream` wait, on the device, for every straggler kernel
- * enqueued so far (the host does not block).  The runs of one generation must be enqueued on one stream.
- * ia_set_pipeline synchronises with the runs in flight; it allocates the queues (IA_ENOMEM). */
+ * trajectory is a serial chain of dependent steps.  With depth 0 (the default) every run finishes on its
+ * own: bulk kernel, then the straggler chain for what it left, both on the caller's stream.  With depth
+ * d > 0 (at most 64) successive runs of the ctx form a pipeline: the bulk kernel of a run hands everything
+ * it still holds when its work counter is empty to the bulk kernel of the NEXT run, which resumes those
+ * trajectories first and then generates its own -- long trajectories keep living in full warps while new
+ * ones keep arriving, and the machine never idles between runs.  Every trajectory in flight carries the
+ * output pointers of the run it belongs to.  Only ia_join ends the pipeline: it enqueues ONE straggler
+ * chain on `cuda_stream` for what the last bulk kernel left (after d runs without a join the next ia_run
+ * does that itself, on its own stream).  The outputs of a pipelined ia_run are therefore complete -- and
+ * its buffers may be released -- only after ia_join; the host does not block in either call.  Runs on
+ * different streams of one ctx are ordered on the device one after the other (they share the ctx's
+ * queues).  ia_set_pipeline blocks until everything in flight on the ctx has finished. */
 int ia_set_pipeline(ia_ctx *ctx, int depth);
 int ia_join(ia_ctx *ctx, void *cuda_stream);
 
 /* Asynchronous form of ia_run_host: enqueues the copies in, the kernels and the copies back on
  * ctx-owned streams and returns; host buffers must be page-locked for the copies to overlap and stay
- * untouched until ia_wait, which blocks the host until every run submitted on this ctx (either way)
- * has finished.  With ia_set_pipeline(d) the submitted runs form generations as above. */
+ * untouched until ia_wait.  With ia_set_pipeline(d) the submitted runs form a pipeline as above: the
+ * records of a run are copied back right behind its bulk kernel, while the next run's bulk kernel works;
+ * the few trajectories (at most one per lane of the grid) that outlive their run's bulk kernel report
+ * through a ctx-owned list which ia_wait copies back and stores into the host arrays.
+ *   ia_sync blocks the host until every kernel and copy enqueued so far has finished, without ending
+ *           the pipeline (trajectories in flight stay in flight; their records and the summaries are not
+ *           final yet).
+ *   ia_wait ends the pipeline (the straggler chain), brings back summaries and late records, and blocks
+ *           until every run submitted on this ctx (either way) has finished.
+ * Blocking and allocation: ia_create, ia_set_pipeline, ia_wait, ia_sync, ia_run_host, ia_get_timing and
+ * ia_destroy block the host.  ia_submit_host blocks only when it has to grow a staging buffer, when
+ * d runs are open or when 64 summaries are pending (it then does an ia_wait first); it allocates
+ * ctx-owned device staging (three buffers of the largest run's size) and, pipelined, a late-record list
+ * in device and page-locked host memory (IA_ENOMEM).  ia_run, ia_join, ia_generate, ia_step_map and
+ * ia_trace never block, allocate or synchronise.  The library reads no environment variables. */
 int ia_submit_host(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *host_outputs);
+int ia_sync(ia_ctx *ctx);
 int ia_wait(ia_ctx *ctx);
 
 /* Generator only (R1-R3): ic_dump is a DEVICE buffer [n][14]. */
@@ -252,11 +271,11 @@ int ia_set_handoff(ia_ctx *ctx, int lanes);
 int ia_set_chain(ia_ctx *ctx, int levels, uint32_t budget);
 
 /* Device times of a run of this ctx, from CUDA events the library records around its kernels: the run's
- * bulk kernel, and the straggler kernel that finished its hand-overs (with a pipeline that kernel is
- * shared by the runs of a generation), in ms.  runs_back = 0 is the most recent run, 1 the one before
- * ...; a run is on record until its generation buffer is used again (depth 0: the latest run only) and
- * once its straggler kernel has been enqueued (IA_EINVAL otherwise).  Synchronises with the end of that
- * run.  Host pointers.  ia_get_last_timing(ctx, ...) = ia_get_timing(ctx, 0, ...). */
+ * bulk kernel, and the straggler chain that ended the pipeline the run was part of (shared by all runs
+ * since the join before; 0 for a run that needed none), in ms.  runs_back = 0 is the most recent run, 1
+ * the one before ...; the last 256 runs and 8 chains are on record, a pipelined run only once its chain
+ * has been enqueued (IA_EINVAL otherwise).  Synchronises with the end of that run.  Host pointers.
+ * ia_get_last_timing(ctx, ...) = ia_get_timing(ctx, 0, ...). */
 int ia_get_timing(ia_ctx *ctx, int runs_back, double *bulk_ms, double *coop_ms);
 int ia_get_last_timing(ia_ctx *ctx, double *bulk_ms, double *coop_ms);
 

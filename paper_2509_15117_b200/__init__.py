@@ -13,16 +13,10 @@ is a small convenience wrapper that owns one ``ia_ctx`` handle.
 from __future__ import annotations
 
 import ctypes as C
-import os
 from pathlib import Path
 from typing import Optional
 
 import numpy as np
-
-# ia_set_pipeline(d) runs up to d straggler kernels on streams of their own; CUDA maps streams onto
-# CUDA_DEVICE_MAX_CONNECTIONS hardware queues (default 8) and streams sharing a queue serialise.  Only
-# effective when set before the process initialises CUDA, hence here at import.
-os.environ.setdefault("CUDA_DEVICE_MAX_CONNECTIONS", "32")
 
 _HERE = Path(__file__).resolve().parent
 LIB_PATH = _HERE / "libia_b200.so"
@@ -38,7 +32,7 @@ IA_STRAGGLER_LEVELS = 12
 # every symbol include/ia.h declares (tests/test_cabi.py checks the library exports each of them)
 EXPORTS = ("ia_create", "ia_run", "ia_run_host", "ia_generate", "ia_step_map", "ia_trace", "ia_get_derived",
            "ia_get_kernel_info", "ia_set_handoff", "ia_set_chain", "ia_get_last_timing", "ia_get_timing", "ia_set_pipeline", "ia_join",
-           "ia_submit_host", "ia_wait", "ia_fp64_peak", "ia_destroy", "ia_strerror", "ia_last_error")
+           "ia_submit_host", "ia_sync", "ia_wait", "ia_fp64_peak", "ia_destroy", "ia_strerror", "ia_last_error")
 
 
 class IaError(RuntimeError):
@@ -83,7 +77,7 @@ SUMMARY_DTYPE = np.dtype([("n_done", "<u8"), ("n_status", "<u8", (5,)), ("n_comp
                           ("sum_ke", "<f8"), ("sum_ke2", "<f8"), ("hist_ncoll", "<u8", (IA_HIST_BINS,)),
                           ("t_first_idle_ns", "<u8"), ("t_start_ns", "<u8"), ("t_end_ns", "<u8"),
                           ("warn", "<u8"), ("n_handoff", "<u8"), ("steps_coop", "<u8"), ("t_bulk_end_ns", "<u8"),
-                          ("slots_bulk", "<u8"), ("reserved", "<u8", (12,)), ("hist_tlife", "<u8", (IA_LIFE_BINS,))])
+                          ("slots_bulk", "<u8"), ("steps_kernel", "<u8"), ("reserved", "<u8", (11,)), ("hist_tlife", "<u8", (IA_LIFE_BINS,))])
 RECORD_BYTES, SUMMARY_BYTES, IC_DUMP_COLS = 64, 1024, 14
 assert RECORD_DTYPE.itemsize == RECORD_BYTES and SUMMARY_DTYPE.itemsize == SUMMARY_BYTES
 
@@ -122,6 +116,7 @@ def load() -> C.CDLL:
     L.ia_join.argtypes = [vp, vp]
     L.ia_submit_host.argtypes = [vp, C.POINTER(ia_launch), C.POINTER(ia_outputs)]
     L.ia_wait.argtypes = [vp]
+    L.ia_sync.argtypes = [vp]
     L.ia_fp64_peak.argtypes = [C.c_int, C.c_double, dp, dp]
     L.ia_destroy.argtypes = [vp]
     L.ia_strerror.argtypes = [C.c_int]
@@ -274,12 +269,12 @@ def ia_get_last_timing(handle) -> dict:
 
 
 def ia_set_pipeline(handle, depth: int) -> None:
-    """Up to `depth` runs finish their longest trajectories on ctx-owned streams while later runs start."""
+    """depth > 0: the bulk kernel of a run resumes what the run before left unfinished; ia_join ends the pipeline."""
     _check(load().ia_set_pipeline(handle, int(depth)), handle)
 
 
 def ia_join(handle, stream=None) -> None:
-    """Makes `stream` (default: torch's current stream) wait on the device for every straggler kernel enqueued."""
+    """Enqueues the straggler chain of the open pipeline on `stream` (default: torch's current stream)."""
     _check(load().ia_join(handle, _stream_handle(stream)), handle)
 
 
@@ -291,6 +286,11 @@ def ia_submit_host(handle, launch: ia_launch, records=None, summary=None, ic_dum
 
 def ia_wait(handle) -> None:
     _check(load().ia_wait(handle), handle)
+
+
+def ia_sync(handle) -> None:
+    """Blocks until every kernel and copy enqueued so far has finished; the pipeline stays open."""
+    _check(load().ia_sync(handle), handle)
 
 
 def ia_fp64_peak(device: int = 0, target_ms: float = 200.0) -> dict:
@@ -360,6 +360,9 @@ class Context:
 
     def wait(self) -> None:
         ia_wait(self.handle)
+
+    def sync(self) -> None:
+        ia_sync(self.handle)
 
     def alloc(self, n: int, ic_dump: bool = False):
         """(records uint8[n*64], summary uint8[1024] zeroed, ic_dump float64[n,14] or None) on the device."""

@@ -23,10 +23,11 @@ struct IaKernelInfo {
     int blocks_per_sm = 0, threads_per_block = 0, regs = 0, local_bytes = 0;
 };
 
-#define IA_PIPE_MAX 64     /* runs per generation */
-#define IA_RUN_RING 128    /* runs whose kernel events are kept for ia_get_timing */
-#define IA_COUNTER_RING 256 /* slots of 4 x u64 */
-#define IA_SCRATCH_WORDS 32
+#define IA_PIPE_MAX 64      /* runs between two joins (ia_set_pipeline) */
+#define IA_RUN_RING 256     /* runs whose kernel events are kept for ia_get_timing */
+#define IA_FLUSH_RING 8     /* straggler chains whose events are kept */
+#define IA_COUNTER_RING 256 /* work counters of the runs that need no queue */
+#define IA_NSTAGE 3         /* device staging buffers of the host entry points */
 
 /* The straggler chain: the cooperative kernel is launched IA_STRAGGLER_LEVELS times in a
  * row.  Level j runs until its queue is empty and then for level_budget << j more iterations per warp; what
@@ -37,60 +38,74 @@ struct IaKernelInfo {
  * trajectory of N steps passes ~log2(N / budget) hand-overs of 256 bytes.  The last level keeps everything. */
 #define IA_BULK_BUDGET 4096u /* the bulk kernel: a warp hands over at the latest this long after the counter ran dry */
 
-/* One run of a generation: what the host entry points have to copy back once its stragglers are done. */
-struct IaPending {
-    ia_outputs host = {nullptr, nullptr, nullptr}; /* host destinations (all NULL for a device-resident run) */
-    ia_outputs dev = {nullptr, nullptr, nullptr};  /* where they sit in the staging */
-    uint64_t n = 0;
-};
-
-/* A generation = the runs whose stragglers ONE launch of the cooperative kernel finishes (ia_set_pipeline).
- * With depth 0 every run is a generation of its own and everything stays on the caller's stream. */
-struct IaGeneration {
-    IaHand *queue = nullptr;        /* hand-over queue shared by the generation's bulk kernels          */
-    size_t queue_cap = 0;           /* in entries                                                       */
-    IaHand *queue2 = nullptr;       /* second queue of the straggler chain (the levels ping-pong)       */
-    unsigned long long *scratch = nullptr; /* per level j: [2j] entries queued for it, [2j+1] its work counter */
-    cudaStream_t tail = nullptr;    /* stream of the cooperative kernel when depth > 0                  */
-    cudaEvent_t ev_coop[2] = {nullptr, nullptr}; /* around the cooperative kernel                        */
-    cudaEvent_t ev_end = nullptr;   /* after it and after the copies back of the host entry points      */
-    bool used = false;              /* ev_end has been recorded                                         */
-    int n_pending = 0;              /* bulk kernels enqueued, cooperative kernel not yet                */
-    unsigned long long serial = 0;  /* counts the generations this buffer has served                    */
-    IaPending pending[IA_PIPE_MAX];
-    int run_idx[IA_PIPE_MAX] = {};  /* their places in the ring of run events                           */
-    cudaStream_t last_stream = nullptr; /* stream of the generation's latest bulk kernel                */
-    void *stage[IA_PIPE_MAX] = {};  /* device staging of the host entry points, per run of the generation */
-    size_t stage_bytes[IA_PIPE_MAX] = {};
-};
+/* Device words of the open pipeline cycle (all zeroed when a cycle starts):
+ *   cnt[k], k = 0..IA_PIPE_MAX: trajectories handed INTO run k of the cycle (cnt[0] stays 0; run k counts what it
+ *                               hands on in cnt[k+1]); cnt[n_open] is what the straggler chain starts from
+ *   wc[k]:                      work counter of run k's bulk kernel
+ *   chain[2j], chain[2j+1]:     level j >= 1 of the chain: trajectories queued for it, its work counter
+ *                               (level 0 uses cnt[n_open] and chain[1])                                   */
+#define IA_W_CNT 0
+#define IA_W_WC (IA_W_CNT + IA_PIPE_MAX + 1)
+#define IA_W_CHAIN (IA_W_WC + IA_PIPE_MAX)
+#define IA_W_TOTAL (IA_W_CHAIN + 2 * IA_STRAGGLER_LEVELS + 2)
 
 struct IaRunEvents {
     cudaEvent_t ev[2] = {nullptr, nullptr}; /* around the bulk kernel */
-    int gen = 0;                            /* generation buffer and its serial at the time: where the  */
-    unsigned long long gen_serial = 0;      /* cooperative-kernel time of this run is found             */
+    long long flush = -1;                   /* id of the straggler chain that finishes the run; -1: none needed */
+};
+
+struct IaFlush {
+    cudaEvent_t ev[2] = {nullptr, nullptr}; /* around the chain */
+    long long id = -1;
+};
+
+struct IaStage {
+    char *buf = nullptr;
+    size_t bytes = 0;
+    cudaEvent_t ev_free = nullptr; /* after the copies back of the run that used it last */
+    bool used = false;
+};
+
+/* A host run whose summary (and late records) ia_wait still has to bring back. */
+struct IaPending {
+    ia_summary *host_summary = nullptr;
+    ia_summary *dev_summary = nullptr;
 };
 
 struct ia_ctx {
     int device = 0;
     IaParams P;
     double derived[16];
-    /* per-launch scratch, a ring so that launches queued behind one another on a stream do not share:
-     * slot = [work counter of the bulk kernel, pad, pad, pad] */
-    unsigned long long *counters = nullptr;
+    unsigned long long *counters = nullptr; /* ring of work counters for runs of one kernel (no queue) */
     unsigned counter_next = 0;
-    size_t queue_cap = 0; /* hand-over entries ONE run can produce: one per lane of a full bulk grid */
+    size_t queue_cap = 0; /* hand-over entries one bulk kernel can produce: one per lane of a full grid */
     int handoff_lanes = 16;
     double w_harm = 0.0;                   /* |q_x| Omega / 2^(3/2): the ion's trap frequency in thermal runs */
     int levels = IA_STRAGGLER_LEVELS;      /* launches of the straggler chain (ia_set_chain) */
     unsigned level_budget = 8192u;         /* iterations of its first level after the queue ran dry */
     int n_sm = 0;
     IaKernelInfo kinfo[2]; /* 0 bulk, 1 cooperative */
-    int depth = 0;          /* runs per generation - 1 ... 0 = every run on its own (see ia_set_pipeline) */
-    int cur = 0;            /* generation buffer the next run joins */
-    IaGeneration gen[2];    /* two, so that the bulk kernels of one generation overlap the stragglers of the last */
-    unsigned long long seq = 0; /* runs launched so far */
+    /* the pipeline (ia_set_pipeline): bulk kernels hand what they leave unfinished to one another through q[0], q[1] */
+    int depth = 0;
+    IaHand *q[2] = {nullptr, nullptr};
+    unsigned long long *words = nullptr; /* IA_W_TOTAL words, see above */
+    int n_open = 0;                      /* bulk kernels enqueued since the last chain */
+    long long flush_next = 0;            /* id of the chain that will finish them */
+    IaFlush flush[IA_FLUSH_RING];
+    cudaEvent_t ev_last = nullptr;       /* after the latest kernel of this ctx: the next run waits for it, */
+    bool ev_last_valid = false;          /* whatever stream it comes in on (the scratch above is shared)    */
+    unsigned long long seq = 0;          /* runs launched so far */
     IaRunEvents run[IA_RUN_RING];
-    cudaStream_t host_stream = nullptr; /* ia_submit_host / ia_run_host */
+    /* host entry points */
+    cudaStream_t host_stream = nullptr, copy_stream = nullptr;
+    IaStage stage[IA_NSTAGE];
+    unsigned stage_next = 0;
+    ia_summary *sum_stage = nullptr;     /* device: one summary per pending host run */
+    IaPending pending[IA_PIPE_MAX];
+    int n_pending = 0;
+    IaLate *late_dev = nullptr, *late_host = nullptr; /* records of late finishers of pipelined host runs */
+    unsigned long long *n_late = nullptr;             /* device counter */
+    unsigned long long late_cap = 0;
     std::string err;
 };
 
@@ -101,28 +116,6 @@ static int fail_cuda(ia_ctx *c, const char *what, cudaError_t e) {
 static int fail_inval(ia_ctx *c, const char *what) {
     if (c) c->err = what;
     return IA_EINVAL;
-}
-
-/* (re)allocates what generation buffer g owns for `runs` runs per generation */
-static cudaError_t gen_init(ia_ctx *c, int g, int runs) {
-    IaGeneration &G = c->gen[g];
-    cudaError_t e = cudaSuccess;
-    const size_t cap = c->queue_cap * (size_t)runs;
-    if (cap > G.queue_cap) {
-        if (G.queue) cudaFree(G.queue);
-        G.queue = nullptr;
-        G.queue_cap = 0;
-        e = cudaMalloc(&G.queue, cap * sizeof(IaHand));
-        if (e == cudaSuccess) G.queue_cap = cap;
-    }
-    if (e == cudaSuccess && !G.queue2)
-        e = cudaMalloc(&G.queue2, (size_t)c->n_sm * c->kinfo[1].blocks_per_sm * 10 * sizeof(IaHand));
-    if (e == cudaSuccess && !G.scratch) e = cudaMalloc(&G.scratch, IA_SCRATCH_WORDS * sizeof(unsigned long long));
-    if (e == cudaSuccess && !G.tail) e = cudaStreamCreateWithFlags(&G.tail, cudaStreamNonBlocking);
-    for (int j = 0; j < 2 && e == cudaSuccess; ++j)
-        if (!G.ev_coop[j]) e = cudaEventCreate(&G.ev_coop[j]);
-    if (e == cudaSuccess && !G.ev_end) e = cudaEventCreate(&G.ev_end);
-    return e;
 }
 
 extern "C" {
@@ -223,12 +216,23 @@ int ia_create(ia_ctx **out, const ia_species *sp, const ia_trap *tr, double De_K
         e = ia_persistent_info(k == 0 ? 1 : 3, &c->kinfo[k].blocks_per_sm, &c->kinfo[k].threads_per_block,
                                &c->kinfo[k].regs, &c->kinfo[k].local_bytes);
     if (e == cudaSuccess) {
+        /* one entry per lane of a full bulk grid (a full cooperative grid holds fewer) */
         c->queue_cap = (size_t)c->n_sm * c->kinfo[0].blocks_per_sm * c->kinfo[0].threads_per_block;
-        e = gen_init(c, 0, 1);
+        for (int j = 0; j < 2 && e == cudaSuccess; ++j) e = cudaMalloc(&c->q[j], c->queue_cap * sizeof(IaHand));
     }
+    if (e == cudaSuccess) e = cudaMalloc(&c->words, IA_W_TOTAL * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMalloc(&c->n_late, sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMemset(c->n_late, 0, sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMalloc(&c->sum_stage, IA_PIPE_MAX * sizeof(ia_summary));
     for (int k = 0; k < IA_RUN_RING && e == cudaSuccess; ++k)
         for (int j = 0; j < 2 && e == cudaSuccess; ++j) e = cudaEventCreate(&c->run[k].ev[j]);
+    for (int k = 0; k < IA_FLUSH_RING && e == cudaSuccess; ++k)
+        for (int j = 0; j < 2 && e == cudaSuccess; ++j) e = cudaEventCreate(&c->flush[k].ev[j]);
+    for (int k = 0; k < IA_NSTAGE && e == cudaSuccess; ++k)
+        e = cudaEventCreateWithFlags(&c->stage[k].ev_free, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_last, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->host_stream, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking);
     if (e != cudaSuccess) {
         const int rc = e == cudaErrorMemoryAllocation ? IA_ENOMEM : IA_ECUDA;
         ia_destroy(c);
@@ -241,26 +245,31 @@ int ia_create(ia_ctx **out, const ia_species *sp, const ia_trap *tr, double De_K
 int ia_destroy(ia_ctx *ctx) {
     if (!ctx) return IA_EINVAL;
     cudaSetDevice(ctx->device);
-    /* runs still in flight finish first: their kernels use the ctx's scratch.  (Bulk kernels whose generation
-     * was never joined are on the caller's stream: the caller synchronises that one.) */
+    /* runs still in flight finish first: their kernels use the ctx's scratch (every kernel of the ctx is
+     * followed by ev_last on its stream; the host entry points' copies are on the ctx's own streams) */
+    if (ctx->ev_last && ctx->ev_last_valid) cudaEventSynchronize(ctx->ev_last);
     if (ctx->host_stream) cudaStreamSynchronize(ctx->host_stream);
-    for (int g = 0; g < 2; ++g) {
-        IaGeneration &G = ctx->gen[g];
-        if (G.used) cudaEventSynchronize(G.ev_end);
-        if (G.tail) cudaStreamDestroy(G.tail);
-        if (G.queue) cudaFree(G.queue);
-        if (G.queue2) cudaFree(G.queue2);
-        if (G.scratch) cudaFree(G.scratch);
-        for (int k = 0; k < IA_PIPE_MAX; ++k)
-            if (G.stage[k]) cudaFree(G.stage[k]);
-        for (int j = 0; j < 2; ++j)
-            if (G.ev_coop[j]) cudaEventDestroy(G.ev_coop[j]);
-        if (G.ev_end) cudaEventDestroy(G.ev_end);
+    if (ctx->copy_stream) cudaStreamSynchronize(ctx->copy_stream);
+    for (int j = 0; j < 2; ++j)
+        if (ctx->q[j]) cudaFree(ctx->q[j]);
+    if (ctx->words) cudaFree(ctx->words);
+    if (ctx->n_late) cudaFree(ctx->n_late);
+    if (ctx->sum_stage) cudaFree(ctx->sum_stage);
+    if (ctx->late_dev) cudaFree(ctx->late_dev);
+    if (ctx->late_host) cudaFreeHost(ctx->late_host);
+    for (int k = 0; k < IA_NSTAGE; ++k) {
+        if (ctx->stage[k].buf) cudaFree(ctx->stage[k].buf);
+        if (ctx->stage[k].ev_free) cudaEventDestroy(ctx->stage[k].ev_free);
     }
+    for (int k = 0; k < IA_FLUSH_RING; ++k)
+        for (int j = 0; j < 2; ++j)
+            if (ctx->flush[k].ev[j]) cudaEventDestroy(ctx->flush[k].ev[j]);
     for (int k = 0; k < IA_RUN_RING; ++k)
         for (int j = 0; j < 2; ++j)
             if (ctx->run[k].ev[j]) cudaEventDestroy(ctx->run[k].ev[j]);
+    if (ctx->ev_last) cudaEventDestroy(ctx->ev_last);
     if (ctx->host_stream) cudaStreamDestroy(ctx->host_stream);
+    if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
     if (ctx->counters) cudaFree(ctx->counters);
     delete ctx;
     return IA_OK;
@@ -303,25 +312,18 @@ int ia_get_timing(ia_ctx *ctx, int runs_back, double *bulk_ms, double *coop_ms) 
     if (runs_back < 0 || runs_back >= IA_RUN_RING || (unsigned long long)runs_back >= ctx->seq)
         return fail_inval(ctx, "ia_get_timing: that run is no longer (or not yet) on record");
     const IaRunEvents &R = ctx->run[(ctx->seq - 1 - (unsigned long long)runs_back) % IA_RUN_RING];
-    if (R.gen < 0) { /* one kernel to the end (IA_PATH_BULK_ONLY / IA_PATH_COOP_ONLY / hand-over off) */
-        cudaError_t e0 = cudaSetDevice(ctx->device);
-        if (e0 == cudaSuccess) e0 = cudaEventSynchronize(R.ev[1]);
-        float a0 = 0.f;
-        if (e0 == cudaSuccess) e0 = cudaEventElapsedTime(&a0, R.ev[0], R.ev[1]);
-        if (e0 != cudaSuccess) return fail_cuda(ctx, "ia_get_timing", e0);
-        *bulk_ms = a0;
-        *coop_ms = 0.0;
-        return IA_OK;
+    const IaFlush *F = nullptr;
+    if (R.flush >= 0) { /* the chain that finished (or will finish) what the run's bulk kernel handed on */
+        if (R.flush >= ctx->flush_next)
+            return fail_inval(ctx, "ia_get_timing: the run's stragglers are not enqueued yet (ia_join)");
+        F = &ctx->flush[R.flush % IA_FLUSH_RING];
+        if (F->id != R.flush) return fail_inval(ctx, "ia_get_timing: that run is no longer on record");
     }
-    const IaGeneration &G = ctx->gen[R.gen];
-    if (G.serial != R.gen_serial + 1 || !G.used)
-        return fail_inval(ctx, G.serial == R.gen_serial ? "ia_get_timing: the run's stragglers are not enqueued yet (ia_join)"
-                                                        : "ia_get_timing: that run is no longer on record");
     cudaError_t e = cudaSetDevice(ctx->device);
-    if (e == cudaSuccess) e = cudaEventSynchronize(G.ev_end);
+    if (e == cudaSuccess) e = cudaEventSynchronize(F ? F->ev[1] : R.ev[1]);
     float a = 0.f, b = 0.f;
     if (e == cudaSuccess) e = cudaEventElapsedTime(&a, R.ev[0], R.ev[1]);
-    if (e == cudaSuccess) e = cudaEventElapsedTime(&b, G.ev_coop[0], G.ev_coop[1]);
+    if (e == cudaSuccess && F) e = cudaEventElapsedTime(&b, F->ev[0], F->ev[1]);
     if (e != cudaSuccess) return fail_cuda(ctx, "ia_get_timing", e);
     *bulk_ms = a;
     *coop_ms = b;
@@ -418,73 +420,73 @@ static int grid_for(const ia_ctx *ctx, int k, unsigned long long n) {
     return (int)(need < full ? need : full);
 }
 
-/* Enqueues the cooperative kernel that finishes the hand-overs of generation buffer g, and the copies back
- * of its host runs.  `st` is the stream the call came in on; with depth 0 everything stays on it. */
-static int flush_generation(ia_ctx *ctx, int g, cudaStream_t st) {
-    IaGeneration &G = ctx->gen[g];
-    if (G.n_pending == 0) return IA_OK;
-    cudaError_t e = cudaSuccess;
-    cudaStream_t ts = st;
-    if (ctx->depth > 0) {
-        /* on the generation's own stream, behind the bulk kernels of all its runs: the caller's stream is free
-         * for the next generation's bulk kernels while this one's longest trajectories finish */
-        ts = G.tail;
-        for (int k = 0; k < G.n_pending && e == cudaSuccess; ++k)
-            e = cudaStreamWaitEvent(ts, ctx->run[G.run_idx[k]].ev[1], 0);
-        if (e != cudaSuccess) return fail_cuda(ctx, "cudaStreamWaitEvent(generation)", e);
-    }
+/* what every persistent kernel of the ctx is told about the late list (records wanted in host arrays) */
+static void sched_late(const ia_ctx *ctx, IaSched *S) {
+    S->late = ctx->late_dev;
+    S->n_late = ctx->n_late;
+    S->late_cap = ctx->late_dev ? ctx->late_cap : 0ull;
+}
+
+/* every kernel of a ctx shares its scratch (queues, counters): a run waits, on the device, for the ctx's latest
+ * kernel whatever stream that one is on */
+static cudaError_t order_after_last(ia_ctx *ctx, cudaStream_t st) {
+    return ctx->ev_last_valid ? cudaStreamWaitEvent(st, ctx->ev_last, 0) : cudaSuccess;
+}
+static cudaError_t mark_last(ia_ctx *ctx, cudaStream_t st) {
+    const cudaError_t e = cudaEventRecord(ctx->ev_last, st);
+    if (e == cudaSuccess) ctx->ev_last_valid = true;
+    return e;
+}
+
+/* Enqueues, on `st`, the straggler chain that finishes what the open runs' bulk kernels left in the queue. */
+static int flush_open(ia_ctx *ctx, cudaStream_t st) {
+    if (ctx->n_open == 0) return IA_OK;
+    cudaError_t e = order_after_last(ctx, st);
+    if (e != cudaSuccess) return fail_cuda(ctx, "cudaStreamWaitEvent(chain)", e);
     IaGen G0;
     std::memset(&G0, 0, sizeof(G0));
     IaOut O0 = {nullptr, nullptr, nullptr}; /* every queue entry carries the outputs of its own run */
-    unsigned long long most = (unsigned long long)G.n_pending * ctx->queue_cap / 32ull *
-                              (unsigned long long)(ctx->handoff_lanes > 0 ? ctx->handoff_lanes : 32);
-    IaHand *q_in = G.queue, *q_out = G.queue2;
-    e = cudaEventRecord(G.ev_coop[0], ts);
+    /* what level 0 may find: every lane of a full bulk grid (a pipelined bulk kernel hands over all it holds),
+     * or the lanes the hand-over threshold lets through */
+    unsigned long long most = ctx->queue_cap;
+    if (ctx->depth == 0 && ctx->handoff_lanes < 32) most = ctx->queue_cap / 32ull * (unsigned long long)ctx->handoff_lanes;
+    int qi = (ctx->n_open - 1) & 1; /* the queue the last bulk kernel wrote */
+    unsigned long long *chain = ctx->words + IA_W_CHAIN;
+    IaFlush &F = ctx->flush[ctx->flush_next % IA_FLUSH_RING];
+    e = cudaEventRecord(F.ev[0], st);
     for (int j = 0; j < ctx->levels && e == cudaSuccess; ++j) {
         IaSched S5;
         std::memset(&S5, 0, sizeof(S5));
-        S5.q_in = q_in;
-        S5.n_in = G.scratch + 2 * j;
-        S5.counter = G.scratch + 2 * j + 1;
+        sched_late(ctx, &S5);
+        S5.q_in = ctx->q[qi];
+        S5.n_in = j == 0 ? ctx->words + IA_W_CNT + ctx->n_open : chain + 2 * j;
+        S5.counter = chain + 2 * j + 1;
         if (j + 1 < ctx->levels) {
-            S5.q_out = q_out;
-            S5.n_out = G.scratch + 2 * (j + 1);
+            S5.q_out = ctx->q[qi ^ 1];
+            S5.n_out = chain + 2 * (j + 1);
             S5.handoff_lanes = 0;
             const unsigned long long b = (unsigned long long)ctx->level_budget << j;
             S5.budget = b > 0xffffffffull ? 0xffffffffu : (unsigned)b;
         }
         const int blocks = grid_for(ctx, 1, most);
-        e = ia_launch_persistent(3, ctx->P, G0, O0, S5, blocks, ts);
+        e = ia_launch_persistent(3, ctx->P, G0, O0, S5, blocks, st);
         most = (unsigned long long)blocks * 10ull; /* what level j can pass on at most: all it holds */
-        IaHand *t = q_in;
-        q_in = q_out;
-        q_out = t;
+        qi ^= 1;
     }
-    if (e == cudaSuccess) e = cudaEventRecord(G.ev_coop[1], ts);
-    for (int k = 0; k < G.n_pending && e == cudaSuccess; ++k) {
-        const IaPending &Q = G.pending[k];
-        if (Q.host.records)
-            e = cudaMemcpyAsync(Q.host.records, Q.dev.records, Q.n * sizeof(ia_record), cudaMemcpyDeviceToHost, ts);
-        if (e == cudaSuccess && Q.host.ic_dump)
-            e = cudaMemcpyAsync(Q.host.ic_dump, Q.dev.ic_dump, Q.n * 14 * sizeof(double), cudaMemcpyDeviceToHost, ts);
-        if (e == cudaSuccess && Q.host.summary)
-            e = cudaMemcpyAsync(Q.host.summary, Q.dev.summary, sizeof(ia_summary), cudaMemcpyDeviceToHost, ts);
-    }
-    if (e == cudaSuccess) e = cudaEventRecord(G.ev_end, ts);
-    if (e != cudaSuccess) return fail_cuda(ctx, "cooperative kernel launch", e);
-    G.used = true;
-    G.serial++;
-    G.n_pending = 0;
-    if (ctx->depth > 0) ctx->cur ^= 1;
+    if (e == cudaSuccess) e = cudaEventRecord(F.ev[1], st);
+    if (e == cudaSuccess) e = mark_last(ctx, st);
+    if (e != cudaSuccess) return fail_cuda(ctx, "straggler chain launch", e);
+    F.id = ctx->flush_next++;
+    ctx->n_open = 0;
     return IA_OK;
 }
 
-/* ia_run proper.  `pend` (may be NULL) describes the copies back a host entry point wants once the run's
- * last kernel is done; *deferred says whether they were left to the generation's flush. */
+/* ia_run proper.  `late_dst` (may be NULL): host array the records of this run are wanted in (a pipelined host
+ * run).  *ridx_out receives the run's place in the ring of run events. */
 static int run_impl(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *outputs, cudaStream_t st,
-                    const IaPending *pend, bool *deferred) {
-    if (deferred) *deferred = false;
+                    ia_record *late_dst, int *ridx_out) {
     ctx->err.clear();
+    if (ridx_out) *ridx_out = -1;
     if (!outputs) return fail_inval(ctx, "outputs is NULL");
     IaGen Gn;
     unsigned long long warn;
@@ -494,70 +496,82 @@ static int run_impl(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *outp
     cudaError_t e = cudaSetDevice(ctx->device);
     if (e != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", e);
     const std::string warn_text = ctx->err;
-    unsigned long long *scratch = ctx->counters + 4 * (size_t)(ctx->counter_next++ % IA_COUNTER_RING);
-    e = cudaMemsetAsync(scratch, 0, 4 * sizeof(unsigned long long), st);
-    if (e != cudaSuccess) return fail_cuda(ctx, "cudaMemsetAsync(counter)", e);
     IaOut O;
     O.records = outputs->records;
     O.summary = outputs->summary;
     O.ic_dump = outputs->ic_dump;
     const bool coop_only = launch->path == IA_PATH_COOP_ONLY;
     const bool handoff = launch->path == IA_PATH_AUTO && ctx->handoff_lanes > 0;
+    const bool piped = handoff && ctx->depth > 0;
+    if (piped && ctx->n_open >= ctx->depth) { /* the pipeline is full: finish what is open first */
+        rc = flush_open(ctx, st);
+        if (rc != IA_OK) return rc;
+    }
+    e = order_after_last(ctx, st);
+    if (e != cudaSuccess) return fail_cuda(ctx, "cudaStreamWaitEvent(previous run)", e);
     IaSched S;
     std::memset(&S, 0, sizeof(S));
-    S.counter = scratch;
+    sched_late(ctx, &S);
     S.warn = warn;
     const int ridx = (int)(ctx->seq % IA_RUN_RING);
     IaRunEvents &R = ctx->run[ridx];
     if (!handoff) {
-        /* one kernel to the end, on the caller's stream: no generation involved */
+        /* one kernel to the end: no queue involved */
+        unsigned long long *wc = ctx->counters + 4 * (size_t)(ctx->counter_next++ % IA_COUNTER_RING);
+        e = cudaMemsetAsync(wc, 0, 4 * sizeof(unsigned long long), st);
+        if (e != cudaSuccess) return fail_cuda(ctx, "cudaMemsetAsync(counter)", e);
+        S.counter = wc;
+        S.n_in = wc + 1; /* stays 0: nothing to resume */
         e = cudaEventRecord(R.ev[0], st);
         if (e == cudaSuccess)
             e = coop_only ? ia_launch_persistent(3, ctx->P, Gn, O, S, grid_for(ctx, 1, Gn.n), st)
                           : ia_launch_persistent(1, ctx->P, Gn, O, S, grid_for(ctx, 0, Gn.n), st);
         if (e == cudaSuccess) e = cudaEventRecord(R.ev[1], st);
+        if (e == cudaSuccess) e = mark_last(ctx, st);
         if (e != cudaSuccess) return fail_cuda(ctx, "persistent kernel launch", e);
-        R.gen = -1;
+        R.flush = -1;
         ctx->seq++;
+        if (ridx_out) *ridx_out = ridx;
         ctx->err = warn_text;
         return IA_OK;
     }
-    const int g = ctx->depth > 0 ? ctx->cur : 0;
-    IaGeneration &G = ctx->gen[g];
-    /* the generation buffer is free again once the cooperative kernel that read it last has ended */
-    if (G.used) {
-        e = cudaStreamWaitEvent(st, G.ev_end, 0);
-        if (e != cudaSuccess) return fail_cuda(ctx, "cudaStreamWaitEvent(generation buffer)", e);
+    const int k = ctx->n_open; /* place in the open cycle */
+    if (k == 0) {
+        e = cudaMemsetAsync(ctx->words, 0, IA_W_TOTAL * sizeof(unsigned long long), st);
+        if (e != cudaSuccess) return fail_cuda(ctx, "cudaMemsetAsync(pipeline words)", e);
     }
-    if (G.n_pending == 0) {
-        e = cudaMemsetAsync(G.scratch, 0, IA_SCRATCH_WORDS * sizeof(unsigned long long), st);
-        if (e != cudaSuccess) return fail_cuda(ctx, "cudaMemsetAsync(generation)", e);
-    }
-    S.q_out = G.queue;
-    S.n_out = G.scratch;
-    S.handoff_lanes = ctx->handoff_lanes;
+    S.counter = ctx->words + IA_W_WC + k;
+    S.q_in = ctx->q[(k & 1) ^ 1];
+    S.n_in = ctx->words + IA_W_CNT + k;
+    S.q_out = ctx->q[k & 1];
+    S.n_out = ctx->words + IA_W_CNT + k + 1;
+    /* pipelined: the next bulk kernel takes over everything this one still holds as soon as its counter is empty */
+    S.handoff_lanes = piped ? 32 : ctx->handoff_lanes;
     S.budget = IA_BULK_BUDGET;
+    S.late_dst = piped ? late_dst : nullptr;
+    /* a full grid whenever trajectories may come in through the queue (their number is known on the device only) */
+    const int blocks = k > 0 ? grid_for(ctx, 0, ~0ull >> 8) : grid_for(ctx, 0, Gn.n);
     e = cudaEventRecord(R.ev[0], st);
-    if (e == cudaSuccess) e = ia_launch_persistent(1, ctx->P, Gn, O, S, grid_for(ctx, 0, Gn.n), st);
+    if (e == cudaSuccess) e = ia_launch_persistent(1, ctx->P, Gn, O, S, blocks, st);
     if (e == cudaSuccess) e = cudaEventRecord(R.ev[1], st);
+    if (e == cudaSuccess) e = mark_last(ctx, st);
     if (e != cudaSuccess) return fail_cuda(ctx, "bulk kernel launch", e);
-    R.gen = g;
-    R.gen_serial = G.serial;
-    G.pending[G.n_pending] = pend ? *pend : IaPending();
-    G.run_idx[G.n_pending] = ridx;
-    G.last_stream = st;
-    G.n_pending++;
+    R.flush = ctx->flush_next;
+    ctx->n_open++;
     ctx->seq++;
-    if (deferred) *deferred = true;
-    if (G.n_pending >= (ctx->depth > 0 ? ctx->depth : 1)) {
-        rc = flush_generation(ctx, g, st);
+    if (ridx_out) *ridx_out = ridx;
+    if (!piped) {
+        rc = flush_open(ctx, st);
         if (rc != IA_OK) return rc;
     }
     ctx->err = warn_text;
     return IA_OK;
 }
 
-/* enqueues one host-buffer run: H2D, kernels, D2H; nothing here waits for the device */
+static int wait_impl(ia_ctx *ctx);
+
+/* enqueues one host-buffer run: H2D, kernels, D2H; nothing here waits for the device unless a buffer has to grow
+ * or the pipeline is full */
 static int submit_host_impl(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *host_out) {
     ctx->err.clear();
     if (!launch || !host_out) return fail_inval(ctx, "launch or outputs is NULL");
@@ -568,46 +582,58 @@ static int submit_host_impl(ia_ctx *ctx, const ia_launch *launch, const ia_outpu
     cudaError_t e = cudaSetDevice(ctx->device);
     if (e != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", e);
     cudaStream_t st = ctx->host_stream;
-    /* the staging belongs to the place the run will take in its generation (runs without a hand-over use the
-     * first place of buffer 0, strictly in stream order) */
     const bool handoff = launch->path == IA_PATH_AUTO && ctx->handoff_lanes > 0;
-    const int g = (handoff && ctx->depth > 0) ? ctx->cur : 0;
-    IaGeneration &G = ctx->gen[g];
-    const int k = handoff ? G.n_pending : 0;
-    /* staging layout: [summary 1024][records n*64][ic_dump n*14*8][y0 n*12*8][phase n*8] */
-    const size_t off_rec = sizeof(ia_summary);
-    const size_t off_ic = off_rec + (host_out->records ? n * sizeof(ia_record) : 0);
+    const bool piped = handoff && ctx->depth > 0;
+    if (ctx->n_pending >= IA_PIPE_MAX || (piped && ctx->n_open >= ctx->depth)) {
+        const int rc = wait_impl(ctx); /* blocks: the summaries and late records of the pending runs come back */
+        if (rc != IA_OK) return rc;
+    }
+    if (piped && host_out->records && !ctx->late_dev) {
+        /* late list: at most one entry per lane of a bulk grid and run */
+        const unsigned long long cap = (unsigned long long)ctx->queue_cap * IA_PIPE_MAX;
+        e = cudaMalloc(&ctx->late_dev, cap * sizeof(IaLate));
+        if (e == cudaSuccess) e = cudaMallocHost(&ctx->late_host, cap * sizeof(IaLate));
+        if (e != cudaSuccess) {
+            if (ctx->late_dev) cudaFree(ctx->late_dev);
+            ctx->late_dev = nullptr;
+            ctx->err = "late-record list allocation failed";
+            return IA_ENOMEM;
+        }
+        ctx->late_cap = cap;
+    }
+    /* staging layout: [records n*64][ic_dump n*14*8][y0 n*12*8][phase n*8]; the summary sits in sum_stage */
+    const size_t off_ic = host_out->records ? n * sizeof(ia_record) : 0;
     const size_t off_y0 = off_ic + (host_out->ic_dump ? n * 14 * sizeof(double) : 0);
     const size_t off_ph = off_y0 + (launch->mode == IA_IC_EXPLICIT ? n * 12 * sizeof(double) : 0);
     const size_t total = off_ph + (launch->mode == IA_IC_EXPLICIT ? n * sizeof(double) : 0);
-    if (total > G.stage_bytes[k]) {
-        /* whatever still reads the old staging finishes first */
-        e = cudaStreamSynchronize(st);
-        if (e == cudaSuccess && G.used) e = cudaEventSynchronize(G.ev_end);
+    IaStage &T = ctx->stage[ctx->stage_next++ % IA_NSTAGE];
+    if (total > T.bytes) {
+        if (T.used) e = cudaEventSynchronize(T.ev_free); /* whatever still reads the old buffer finishes first */
         if (e != cudaSuccess) return fail_cuda(ctx, "synchronise before staging reallocation", e);
-        if (G.stage[k]) cudaFree(G.stage[k]);
-        G.stage[k] = nullptr;
-        G.stage_bytes[k] = 0;
-        e = cudaMalloc(&G.stage[k], total);
+        if (T.buf) cudaFree(T.buf);
+        T.buf = nullptr;
+        T.bytes = 0;
+        e = cudaMalloc(&T.buf, total);
         if (e != cudaSuccess) {
             ctx->err = "device staging allocation failed";
             return IA_ENOMEM;
         }
-        G.stage_bytes[k] = total;
+        T.bytes = total;
     }
-    if (G.used) { /* the copies back of the generation that used this staging last are behind ev_end */
-        e = cudaStreamWaitEvent(st, G.ev_end, 0);
+    if (T.used) { /* the copies back of the run that used this staging last */
+        e = cudaStreamWaitEvent(st, T.ev_free, 0);
         if (e != cudaSuccess) return fail_cuda(ctx, "cudaStreamWaitEvent(staging)", e);
     }
-    char *base = (char *)G.stage[k];
+    char *base = T.buf;
     ia_launch L = *launch;
-    IaPending Q;
-    Q.host = *host_out;
-    Q.n = n;
-    Q.dev.summary = (ia_summary *)base;
-    Q.dev.records = host_out->records ? (ia_record *)(base + off_rec) : nullptr;
-    Q.dev.ic_dump = host_out->ic_dump ? (double *)(base + off_ic) : nullptr;
-    e = cudaMemsetAsync(base, 0, sizeof(ia_summary), st);
+    ia_outputs dev;
+    IaPending &Q = ctx->pending[ctx->n_pending];
+    Q.host_summary = host_out->summary;
+    Q.dev_summary = ctx->sum_stage + ctx->n_pending;
+    dev.summary = Q.dev_summary;
+    dev.records = host_out->records ? (ia_record *)base : nullptr;
+    dev.ic_dump = host_out->ic_dump ? (double *)(base + off_ic) : nullptr;
+    e = cudaMemsetAsync(dev.summary, 0, sizeof(ia_summary), st);
     if (e != cudaSuccess) return fail_cuda(ctx, "cudaMemsetAsync(summary)", e);
     if (launch->mode == IA_IC_EXPLICIT) {
         e = cudaMemcpyAsync(base + off_y0, launch->y0, n * 12 * sizeof(double), cudaMemcpyHostToDevice, st);
@@ -617,19 +643,54 @@ static int submit_host_impl(ia_ctx *ctx, const ia_launch *launch, const ia_outpu
         L.y0 = (const double *)(base + off_y0);
         L.phase = (const double *)(base + off_ph);
     }
-    bool deferred = false;
-    int rc = run_impl(ctx, &L, &Q.dev, st, &Q, &deferred);
-    if (rc != IA_OK || deferred) return rc;
-    /* no hand-over: the run ended on st, the copies back follow it there */
+    int ridx = -1;
+    int rc = run_impl(ctx, &L, &dev, st, host_out->records, &ridx);
+    if (rc != IA_OK) return rc;
     const std::string warn_text = ctx->err;
-    if (Q.host.records)
-        e = cudaMemcpyAsync(Q.host.records, Q.dev.records, n * sizeof(ia_record), cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess && Q.host.ic_dump)
-        e = cudaMemcpyAsync(Q.host.ic_dump, Q.dev.ic_dump, n * 14 * sizeof(double), cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess && Q.host.summary)
-        e = cudaMemcpyAsync(Q.host.summary, Q.dev.summary, sizeof(ia_summary), cudaMemcpyDeviceToHost, st);
+    ctx->n_pending++;
+    /* Records and initial conditions go back as soon as the run's own kernels are done -- for a pipelined run on the
+     * copy stream, behind its bulk kernel, while the next run's bulk kernel starts; the trajectories that one carries
+     * on report through the late list (ia_wait).  The summary is final only after the chain: ia_wait copies it. */
+    cudaStream_t cs = piped ? ctx->copy_stream : st;
+    if (piped) e = cudaStreamWaitEvent(cs, ctx->run[ridx].ev[1], 0);
+    if (e == cudaSuccess && host_out->records)
+        e = cudaMemcpyAsync(host_out->records, dev.records, n * sizeof(ia_record), cudaMemcpyDeviceToHost, cs);
+    if (e == cudaSuccess && host_out->ic_dump)
+        e = cudaMemcpyAsync(host_out->ic_dump, dev.ic_dump, n * 14 * sizeof(double), cudaMemcpyDeviceToHost, cs);
+    if (e == cudaSuccess) e = cudaEventRecord(T.ev_free, cs);
     if (e != cudaSuccess) return fail_cuda(ctx, "D2H copy", e);
+    T.used = true;
     ctx->err = warn_text;
+    return IA_OK;
+}
+
+/* ia_wait proper: chain of the open runs, summaries and late records of the pending host runs, host blocks */
+static int wait_impl(ia_ctx *ctx) {
+    cudaError_t e = cudaSetDevice(ctx->device);
+    if (e != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", e);
+    cudaStream_t st = ctx->host_stream;
+    int rc = flush_open(ctx, st);
+    if (rc != IA_OK) return rc;
+    e = order_after_last(ctx, st);
+    for (int k = 0; k < ctx->n_pending && e == cudaSuccess; ++k)
+        if (ctx->pending[k].host_summary)
+            e = cudaMemcpyAsync(ctx->pending[k].host_summary, ctx->pending[k].dev_summary, sizeof(ia_summary),
+                                cudaMemcpyDeviceToHost, st);
+    unsigned long long n_late = 0;
+    if (e == cudaSuccess && ctx->late_dev) {
+        e = cudaMemcpyAsync(&n_late, ctx->n_late, sizeof(n_late), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (n_late > ctx->late_cap) n_late = ctx->late_cap; /* cannot happen: one entry per lane and run */
+        if (e == cudaSuccess && n_late > 0)
+            e = cudaMemcpyAsync(ctx->late_host, ctx->late_dev, n_late * sizeof(IaLate), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaMemsetAsync(ctx->n_late, 0, sizeof(unsigned long long), st);
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->copy_stream);
+    if (e != cudaSuccess) return fail_cuda(ctx, "ia_wait", e);
+    /* the records of the trajectories that outlived their run's bulk kernel: stored over what the early copy left */
+    for (unsigned long long k = 0; k < n_late; ++k) *ctx->late_host[k].dst = ctx->late_host[k].rec;
+    ctx->n_pending = 0;
     return IA_OK;
 }
 
@@ -645,12 +706,9 @@ int ia_join(ia_ctx *ctx, void *cuda_stream) {
     cudaStream_t st = (cudaStream_t)cuda_stream;
     cudaError_t e = cudaSetDevice(ctx->device);
     if (e != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", e);
-    for (int g = 0; g < 2; ++g) {
-        const int rc = flush_generation(ctx, g, st);
-        if (rc != IA_OK) return rc;
-    }
-    for (int g = 0; g < 2 && e == cudaSuccess; ++g)
-        if (ctx->gen[g].used) e = cudaStreamWaitEvent(st, ctx->gen[g].ev_end, 0);
+    const int rc = flush_open(ctx, st);
+    if (rc != IA_OK) return rc;
+    e = order_after_last(ctx, st);
     if (e != cudaSuccess) return fail_cuda(ctx, "ia_join", e);
     return IA_OK;
 }
@@ -658,24 +716,10 @@ int ia_join(ia_ctx *ctx, void *cuda_stream) {
 int ia_set_pipeline(ia_ctx *ctx, int depth) {
     if (!ctx) return IA_EINVAL;
     if (depth < 0 || depth > IA_PIPE_MAX) return fail_inval(ctx, "ia_set_pipeline: depth must be in [0, 64]");
-    cudaError_t e = cudaSetDevice(ctx->device);
-    if (e != cudaSuccess) return fail_cuda(ctx, "cudaSetDevice", e);
-    /* runs in flight keep the old layout: enqueue what is pending and let everything finish */
-    for (int g = 0; g < 2; ++g) {
-        const int rc = flush_generation(ctx, g, ctx->gen[g].last_stream);
-        if (rc != IA_OK) return rc;
-    }
-    for (int g = 0; g < 2 && e == cudaSuccess; ++g)
-        if (ctx->gen[g].used) e = cudaEventSynchronize(ctx->gen[g].ev_end);
-    if (e == cudaSuccess) e = gen_init(ctx, 0, depth > 0 ? depth : 1);
-    if (e == cudaSuccess && depth > 0) e = gen_init(ctx, 1, depth);
-    if (e == cudaErrorMemoryAllocation) {
-        ctx->err = "ia_set_pipeline: hand-over queue allocation failed";
-        return IA_ENOMEM;
-    }
-    if (e != cudaSuccess) return fail_cuda(ctx, "ia_set_pipeline", e);
+    /* runs in flight keep the old setting: finish what is open */
+    const int rc = wait_impl(ctx);
+    if (rc != IA_OK) return rc;
     ctx->depth = depth;
-    ctx->cur = 0;
     return IA_OK;
 }
 
@@ -684,13 +728,19 @@ int ia_submit_host(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *host_
     return submit_host_impl(ctx, launch, host_outputs);
 }
 
+int ia_sync(ia_ctx *ctx) {
+    if (!ctx) return IA_EINVAL;
+    cudaError_t e = cudaSetDevice(ctx->device);
+    if (e == cudaSuccess && ctx->ev_last_valid) e = cudaEventSynchronize(ctx->ev_last);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->host_stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->copy_stream);
+    if (e != cudaSuccess) return fail_cuda(ctx, "ia_sync", e);
+    return IA_OK;
+}
+
 int ia_wait(ia_ctx *ctx) {
     if (!ctx) return IA_EINVAL;
-    int rc = ia_join(ctx, ctx->host_stream);
-    if (rc != IA_OK) return rc;
-    cudaError_t e = cudaStreamSynchronize(ctx->host_stream);
-    if (e != cudaSuccess) return fail_cuda(ctx, "ia_wait", e);
-    return IA_OK;
+    return wait_impl(ctx);
 }
 
 int ia_run_host(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *host_outputs) {
@@ -698,7 +748,7 @@ int ia_run_host(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *host_out
     int rc = submit_host_impl(ctx, launch, host_outputs);
     if (rc != IA_OK) return rc;
     const std::string warn_text = ctx->err;
-    rc = ia_wait(ctx);
+    rc = wait_impl(ctx);
     if (rc == IA_OK) ctx->err = warn_text;
     return rc;
 }

@@ -2,7 +2,7 @@
  * ia_kernels.cu -- the persistent propagation kernels (K1 bulk, K5 straggler), the initial-condition
  * generator (K2) and the verification kernels (K3).  Compiled with -fmad=false: see ia_dev.cuh.
  *
- * ia_persistent_kernel<LPT, RESUME>: state, accelerations of all seven stages and step size live in
+ * ia_persistent_kernel<LPT, SRC>: state, accelerations of all seven stages and step size live in
  * registers, what is touched only when a trajectory starts, bounces or ends in one shared-memory struct;
  * nothing per step touches global memory.  A group of LPT lanes owns one trajectory.  A group whose
  * trajectory has terminated writes its 64-byte record, adds to the ensemble summary and takes the next
@@ -12,14 +12,18 @@
  * The step loop proper is an inner loop of up to IA_INNER attempts that is left when a trajectory of the
  * warp terminates; counter, queue and budget logic sit outside it and out of its registers.
  *
- *   K1 = <1, false>: one lane per trajectory, the throughput layout; generates its trajectories.  Once the
- *        work counter is empty and a warp is down to `handoff_lanes` running lanes (or `budget` attempts
- *        later at the latest) it writes their states to a queue and exits.
- *   K5 = <3, true>: three lanes per trajectory (x/y/z split); resumes trajectories from a queue.  A third
- *        of the FP64 instructions per lane and step: what counts for the longest trajectories is the
+ *   K1 = <1, IA_SRC_BOTH>: one lane per trajectory, the throughput layout.  Its work counter first deals out
+ *        the trajectories an earlier bulk kernel left unfinished (a hand-over queue; empty for a run on its
+ *        own), then the indices of its own launch, which it generates.  Once the counter is empty and a warp
+ *        is down to `handoff_lanes` running lanes (or `budget` attempts later at the latest) it writes their
+ *        states to a queue and exits.  With ia_set_pipeline that queue feeds the bulk kernel of the NEXT run
+ *        (handoff_lanes = 32: at once), so a trajectory of 10^7 steps lives in full warps across many runs
+ *        and only the last run of a stream is followed by a straggler chain.
+ *   K5 = <3, IA_SRC_QUEUE>: three lanes per trajectory (x/y/z split); resumes trajectories from a queue.  A
+ *        third of the FP64 instructions per lane and step: what counts for the longest trajectories is the
  *        latency of one step.  Launched as a chain of levels (ia_api.cu): each level passes what still runs
  *        after its budget to the next, which deals it out ten to a warp again.
- *   <3, false>: the cooperative layout from the first step (IA_PATH_COOP_ONLY, verification).
+ *   <3, IA_SRC_GEN>: the cooperative layout from the first step (IA_PATH_COOP_ONLY, verification).
  * All run the same arithmetic (ia_dev.cuh) and give bit-identical trajectories, so where a trajectory is
  * handed over does not show in its result.
  */
@@ -179,10 +183,12 @@ __device__ __forceinline__ void ia_park(const IaLane<LPT> &L, IaVec<LPT> &Y) {
 
 /* ---- K1 / K5 ---------------------------------------------------------------------------------- */
 
-/* RESUME: the kernel takes its trajectories from a hand-over queue (a level of the straggler chain) instead of
- * generating them; a compile-time switch, so that the chain's kernel carries neither the generator nor its
- * registers -- the latency of its step loop is what the longest trajectories of a launch wait for. */
-template <int LPT, bool RESUME>
+/* SRC says where the kernel's trajectories come from (ia_kernels.cuh): IA_SRC_QUEUE = a level of the straggler
+ * chain, which only resumes what a queue holds -- a compile-time switch, so that the chain's kernel carries neither
+ * the generator nor its registers: the latency of its step loop is what the longest trajectories of a launch wait
+ * for.  IA_SRC_BOTH = the bulk kernel: it first resumes what the bulk kernel of the run before left unfinished
+ * (ia_set_pipeline: long trajectories keep living in full warps while fresh ones keep arriving), then generates. */
+template <int LPT, int SRC>
 __global__ void __launch_bounds__(IA_THREADS, LPT == 1 ? 12 : 16)
 ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__ IaGen G, const IaOut O,
                      const IaSched S) {
@@ -202,6 +208,8 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
         ia_summary *sum[IA_THREADS];
         unsigned steps_in[IA_THREADS], n_coll[IA_THREADS], n_tp[IA_THREADS], n_loc[IA_THREADS], steps_rej[IA_THREADS],
             cnt[IA_THREADS], wexh[IA_THREADS], iters[IA_THREADS];
+        unsigned flags[IA_THREADS];       /* IA_HAND_LATE | IA_CARRIED */
+        unsigned steps_entry[IA_THREADS]; /* attempted steps the trajectory had taken when this kernel got it */
         double loc_lo[IA_THREADS], loc_hi[IA_THREADS]; /* bracket of the exit localisation (R7) */
         double r2_cur[IA_THREADS];                     /* |d|^2 at the current (last committed) state */
     } sh;
@@ -218,13 +226,15 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
     cnt = 0;
     unsigned &iters = sh.iters[threadIdx.x]; /* warp-uniform: step attempts of this warp so far */
     iters = 0;
+    unsigned &flags = sh.flags[threadIdx.x], &steps_entry = sh.steps_entry[threadIdx.x];
+    flags = 0; steps_entry = 0;
     t_first = 0.0; t_last = 0.0; slot = 0; steps_in = 0; n_coll = 0; n_tp = 0; n_loc = 0; steps_rej = 0;
     int mode = MODE_IDLE;
     bool failed = false;
     unsigned &wexh = sh.wexh[threadIdx.x]; /* warp-uniform flag: the work counter is empty */
     wexh = 0u;
     ia_park<LPT>(L, Y);
-    if (!RESUME && O.summary != nullptr && threadIdx.x == 0) {
+    if (SRC != IA_SRC_QUEUE && O.summary != nullptr && threadIdx.x == 0) {
         const unsigned long long t0 = ia_globaltimer();
         if (blockIdx.x == 0) {
             atomicCAS((unsigned long long *)&O.summary->t_start_ns, 0ull, t0);
@@ -236,9 +246,11 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
     /* A kernel that resumes from a queue deals the first gridDim.x * PER_WARP entries out by block index, so that
      * when the queue is short the work sits in the lowest-numbered blocks -- which the hardware spreads over the
      * SMs -- instead of wherever the race for the counter ends; the counter serves the rest of the queue. */
-    constexpr bool resume = RESUME;
+    constexpr bool resume = (SRC == IA_SRC_QUEUE);
+#define IA_CARRIED 2u /* flags: the trajectory came out of a hand-over queue */
 #define IA_DEALT (resume ? (unsigned long long)gridDim.x * PER_WARP : 0ull)
-#define IA_N_TOTAL (resume ? *S.n_in : G.n) /* final: the producer kernel has ended */
+#define IA_N_IN (SRC == IA_SRC_GEN ? 0ull : *S.n_in) /* final: the producer kernel has ended */
+#define IA_N_TOTAL (resume ? IA_N_IN : IA_N_IN + G.n)
     bool first_refill = resume;
 
     for (;;) {
@@ -257,15 +269,16 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
                 base = __shfl_sync(IA_FULL, base, first);
             }
             const unsigned long long j = base + __popc(wm & ((1u << L.gbase) - 1u));
-            const bool got = want && (j < IA_N_TOTAL);
+            const unsigned long long n_in = IA_N_IN;
+            const bool got = want && (j < (resume ? n_in : n_in + G.n));
             if (__any_sync(IA_FULL, want && !got)) {
                 if (!wexh && O.summary != nullptr && !resume && lane == 0)
                     atomicCAS((unsigned long long *)&O.summary->t_first_idle_ns, 0ull, ia_globaltimer());
                 wexh = 1u;
             }
             if (got) {
-                if (resume) {
-                    /* resume a trajectory the bulk kernel handed over */
+                if (resume || (SRC == IA_SRC_BOTH && j < n_in)) {
+                    /* resume a trajectory an earlier kernel handed over */
                     const IaHand *H = S.q_in + j;
 #pragma unroll
                     for (int a = 0; a < NA; ++a) {
@@ -281,13 +294,16 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
                     n_per = H->n_per; n_coll = H->n_coll; n_tp = H->n_tp;
                     steps_acc = H->steps_acc; steps_rej = H->steps_rej; failed = H->failed != 0u;
                     steps_in = H->steps_in;
+                    flags = (H->flags & IA_HAND_LATE) | IA_CARRIED;
+                    steps_entry = steps_acc + steps_rej;
                     n_loc = 0;
                     mode = MODE_RUN;
-                } else {
+                } else if (SRC != IA_SRC_QUEUE) {
+                    const unsigned long long jf = j - n_in; /* index within this launch */
                     IaIC ic;
-                    ia_generate_ic(P, G, j, &ic);
+                    ia_generate_ic(P, G, jf, &ic);
                     if (O.ic_dump != nullptr && L.leader) {
-                        double *o = O.ic_dump + j * 14;
+                        double *o = O.ic_dump + jf * 14;
 #pragma unroll
                         for (int i = 0; i < 6; ++i) {
                             o[i] = ic.x[i];
@@ -296,8 +312,9 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
                         o[12] = ic.phase;
                         o[13] = ic.E_au;
                     }
-                    slot = j;
+                    slot = jf;
                     out_rec = O.records; out_sum = O.summary;
+                    flags = 0; steps_entry = 0;
                     tf = 0.0; n_per = 0; n_coll = 0; n_tp = 0; steps_acc = 0; steps_rej = 0; n_loc = 0; steps_in = 0;
                     t_first = 0.0; t_last = 0.0; failed = false;
                     phase = ic.phase;
@@ -313,7 +330,7 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
                                 r.t_dwell = 0.0; r.t_life = 0.0;
                                 r.va_f[0] = ic.v[3]; r.va_f[1] = ic.v[4]; r.va_f[2] = ic.v[5];
                                 r.n_coll = 0; r.n_tp = 0; r.steps_acc = 0; r.steps_rej = 0; r.status = 3; r.n_loc = 0;
-                                O.records[j] = r;
+                                O.records[jf] = r;
                             }
                             if (O.summary != nullptr) {
                                 atomicAdd((unsigned long long *)&O.summary->n_done, 1ull);
@@ -394,14 +411,22 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
                         H->A1[ax] = Y.Ai[a]; H->A1[3 + ax] = Y.Aa[a];
                     }
                     if (L.leader) {
+                        const bool carried = (flags & IA_CARRIED) != 0u;
                         H->tf = tf; H->h = h; H->phase = phase; H->s_old = s_old;
                         H->r2_cur = sh.r2_cur[threadIdx.x];
                         H->t_first = t_first; H->t_last = t_last; H->slot = slot;
-                        H->records = out_rec; H->summary = out_sum;
+                        /* a trajectory of a pipelined host run leaves with the HOST address of its record array */
+                        const bool to_host = !carried && S.late_dst != nullptr;
+                        H->records = to_host ? S.late_dst : out_rec;
+                        H->flags = to_host ? IA_HAND_LATE : (flags & IA_HAND_LATE);
+                        H->summary = out_sum;
                         H->n_per = n_per; H->n_coll = n_coll; H->n_tp = n_tp;
                         H->steps_acc = steps_acc; H->steps_rej = steps_rej; H->failed = failed ? 1u : 0u;
-                        /* steps taken before the first hand-over (the bulk kernel's share of the trajectory) */
-                        H->steps_in = (resume) ? steps_in : steps_acc + steps_rej;
+                        /* steps taken before the first hand-over */
+                        H->steps_in = carried ? steps_in : steps_acc + steps_rej;
+                        if (SRC != IA_SRC_QUEUE && O.summary != nullptr)
+                            atomicAdd((unsigned long long *)&O.summary->steps_kernel,
+                                      (unsigned long long)(steps_acc + steps_rej - steps_entry));
                     }
                     mode = MODE_IDLE;
                 }
@@ -553,6 +578,7 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
             if (fin >= 0) {
                 if (L.leader) {
                     const double ke = (0.5 * P.m_i) * ia_dot3<true>(VI, VI);
+                    const bool carried = (flags & IA_CARRIED) != 0u;
                     if (out_rec != nullptr) {
                         ia_record r;
                         r.ke_ion = ke;
@@ -565,8 +591,19 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
                         r.steps_rej = (uint16_t)min(steps_rej, 65535u);
                         r.status = (uint8_t)fin;
                         r.n_loc = (uint8_t)n_loc;
-                        out_rec[slot] = r;
+                        if (flags & IA_HAND_LATE) {
+                            const unsigned long long k = atomicAdd(S.n_late, 1ull);
+                            if (k < S.late_cap) {
+                                S.late[k].rec = r;
+                                S.late[k].dst = out_rec + slot;
+                            }
+                        } else {
+                            out_rec[slot] = r;
+                        }
                     }
+                    if (SRC != IA_SRC_QUEUE && O.summary != nullptr)
+                        atomicAdd((unsigned long long *)&O.summary->steps_kernel,
+                                  (unsigned long long)(steps_acc + steps_rej + n_loc - steps_entry));
                     if (out_sum != nullptr) {
                         ia_summary *Sm = out_sum;
                         atomicAdd((unsigned long long *)&Sm->n_done, 1ull);
@@ -575,7 +612,7 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
                         atomicAdd((unsigned long long *)&Sm->steps_acc, (unsigned long long)steps_acc);
                         atomicAdd((unsigned long long *)&Sm->steps_rej, (unsigned long long)steps_rej);
                         atomicAdd((unsigned long long *)&Sm->steps_loc, (unsigned long long)n_loc);
-                        if (resume) {
+                        if (carried) {
                             atomicMax((unsigned long long *)&Sm->t_end_ns, ia_globaltimer());
                             atomicAdd((unsigned long long *)&Sm->n_handoff, 1ull);
                             atomicAdd((unsigned long long *)&Sm->steps_coop,
@@ -697,20 +734,20 @@ __global__ void ia_trace_kernel(const __grid_constant__ IaParams P, IaY12 y0, do
 cudaError_t ia_launch_persistent(int lanes_per_traj, const IaParams &P, const IaGen &G, const IaOut &O,
                                  const IaSched &S, int grid_blocks, cudaStream_t st) {
     if (lanes_per_traj == 1) {
-        if (S.q_in != nullptr) return cudaErrorInvalidValue; /* only the cooperative kernel resumes from a queue */
-        ia_persistent_kernel<1, false><<<grid_blocks, IA_THREADS, 0, st>>>(P, G, O, S);
+        if (S.n_in == nullptr) return cudaErrorInvalidValue; /* the bulk kernel always looks at a queue length */
+        ia_persistent_kernel<1, IA_SRC_BOTH><<<grid_blocks, IA_THREADS, 0, st>>>(P, G, O, S);
     } else if (S.q_in != nullptr) {
-        ia_persistent_kernel<3, true><<<grid_blocks, IA_THREADS, 0, st>>>(P, G, O, S);
+        ia_persistent_kernel<3, IA_SRC_QUEUE><<<grid_blocks, IA_THREADS, 0, st>>>(P, G, O, S);
     } else {
-        ia_persistent_kernel<3, false><<<grid_blocks, IA_THREADS, 0, st>>>(P, G, O, S);
+        ia_persistent_kernel<3, IA_SRC_GEN><<<grid_blocks, IA_THREADS, 0, st>>>(P, G, O, S);
     }
     return cudaGetLastError();
 }
 
 cudaError_t ia_persistent_info(int lanes_per_traj, int *blocks_per_sm, int *threads_per_block, int *regs,
                                int *local_bytes) {
-    const void *fn = lanes_per_traj == 1 ? (const void *)ia_persistent_kernel<1, false>
-                                         : (const void *)ia_persistent_kernel<3, true>;
+    const void *fn = lanes_per_traj == 1 ? (const void *)ia_persistent_kernel<1, IA_SRC_BOTH>
+                                         : (const void *)ia_persistent_kernel<3, IA_SRC_QUEUE>;
     cudaFuncAttributes fa;
     cudaError_t e = cudaFuncGetAttributes(&fa, fn);
     if (e != cudaSuccess) return e;

@@ -28,7 +28,17 @@ struct IaOut {
     double *ic_dump;
 };
 
-/* A trajectory in flight, as the bulk kernel hands it to the straggler kernel (256 bytes). */
+/* A finished trajectory whose home record array is HOST memory (a pipelined host run, ia_submit_host): the kernel
+ * appends the record and its destination to a ctx-owned list, ia_wait copies the list back and stores every record. */
+struct IaLate {
+    ia_record rec;
+    ia_record *dst; /* host address */
+};
+static_assert(sizeof(IaLate) == 72, "IaLate is 72 bytes");
+
+#define IA_HAND_LATE 1u /* IaHand.flags: `records` is a host array, the record goes to the late list */
+
+/* A trajectory in flight, as a kernel hands it to the next one (256 bytes). */
 struct IaHand {
     double x[6], v[6], A1[6]; /* r_i, r_a | v_i, v_a | FSAL accelerations */
     double tf, h, phase, s_old, t_first, t_last;
@@ -37,7 +47,7 @@ struct IaHand {
     ia_record *records;  /* where its outcome goes: the outputs of the run it came from, so that one straggler */
     ia_summary *summary; /* kernel can finish the hand-overs of several runs (ia_set_pipeline)                */
     unsigned steps_in;   /* attempted steps before the first hand-over */
-    unsigned pad32;
+    unsigned flags;      /* IA_HAND_LATE */
     double r2_cur;       /* |d|^2 at the current state (decides whether an exit can be localised, R7) */
 };
 static_assert(sizeof(IaHand) == 256, "IaHand is 256 bytes");
@@ -45,14 +55,25 @@ static_assert(sizeof(IaHand) == 256, "IaHand is 256 bytes");
 /* where a persistent kernel takes its work from and where unfinished work goes */
 struct IaSched {
     unsigned long long *counter;     /* work counter of this launch (zeroed by the host)                 */
-    const IaHand *q_in;              /* non-NULL: resume trajectories from this queue instead of generating */
+    const IaHand *q_in;              /* non-NULL: resume the trajectories of this queue (a level of the straggler
+                                        chain: only those; the bulk kernel: those first, then it generates its own) */
     const unsigned long long *n_in;  /* ... their number (device memory, written by the producing kernel) */
     IaHand *q_out;                   /* non-NULL: hand unfinished trajectories over to this queue ...     */
     unsigned long long *n_out;       /* ... counting them here                                           */
     int handoff_lanes;               /* ... once the counter is empty and <= this many trajectories of a warp run */
     unsigned budget;                 /* ... or once it has run this many iterations since the counter ran dry */
     unsigned long long warn;
+    IaLate *late;                    /* list of finished trajectories whose records live on the host ...  */
+    unsigned long long *n_late;      /* ... its length ...                                                */
+    unsigned long long late_cap;     /* ... and capacity                                                  */
+    ia_record *late_dst;             /* non-NULL: the records of THIS run's trajectories are wanted in this host
+                                        array: a trajectory handed over carries it instead of O.records   */
 };
+
+/* where a persistent kernel's trajectories come from */
+enum { IA_SRC_GEN = 0,   /* the generator (a2)                                                            */
+       IA_SRC_QUEUE = 1, /* a hand-over queue, dealt out by block index (a level of the straggler chain)  */
+       IA_SRC_BOTH = 2 };/* a hand-over queue first, then the generator (the bulk kernel)                 */
 
 /* persistent propagation kernels: lanes_per_traj = 1 (bulk) or 3 (straggler / cooperative layout) */
 cudaError_t ia_launch_persistent(int lanes_per_traj, const IaParams &P, const IaGen &G, const IaOut &O,

@@ -31,7 +31,7 @@ def shard_launch(launch, rank: int, world: int):
 
 
 _SUM_FIELDS = ("n_done", "n_status", "n_complex", "steps_acc", "steps_rej", "steps_loc", "sum_ke", "sum_ke2",
-               "hist_ncoll", "hist_tlife", "slots_bulk", "n_handoff", "steps_coop")
+               "hist_ncoll", "hist_tlife", "slots_bulk", "n_handoff", "steps_coop", "steps_kernel")
 
 
 def summary_to_vector(summary) -> np.ndarray:
@@ -78,3 +78,23 @@ def all_reduce_max(value: float, device=None) -> float:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         return float(t.item())
     return float(value)
+
+
+def all_reduce_sum(value: float, device=None) -> float:
+    import torch
+    import torch.distributed as dist
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        t = torch.tensor([float(value)], dtype=torch.float64)
+        if device is not None:
+            t = t.to(device)
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        return float(t.item())
+    return float(value)
+
+
+def sum_summaries(arr: np.ndarray) -> np.ndarray:
+    """Field-wise sum of an array of ia_summary records (host arithmetic on counters, for reporting)."""
+    out = np.zeros((), dtype=arr.dtype)
+    for f in arr.dtype.names:
+        out[f] = arr[f].sum(axis=0)
+    return out

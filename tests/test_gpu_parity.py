@@ -192,19 +192,22 @@ def _assert_records_identical(a, b):
         assert np.array_equal(a[f], b[f]), f
 
 
-@pytest.mark.parametrize("which", ["config0", "config1", "config4"])
+@pytest.mark.parametrize("which", ["config0", "config1", "config4", "config4_big"])
 def test_bulk_coop_and_handoff_paths_are_bit_identical(P, which):
     """IA_PATH_BULK_ONLY (one lane per trajectory to the end), IA_PATH_COOP_ONLY (three lanes per trajectory
-    from the first step) and IA_PATH_AUTO with hand-over thresholds 4, 16 and 32 lanes: identical records,
-    chaotic trajectories included (config 1 at 48x48 = 2,304 trajectories, a ragged 72 warps; config 4's
-    Philox stream)."""
+    from the first step), IA_PATH_AUTO with hand-over thresholds 4, 16 and 32 lanes, and the pipelined path
+    (ia_set_pipeline: the launch cut into three runs, the bulk kernel of a run resuming what the one before left):
+    identical records, chaotic trajectories included (config 1 at 48x48 = 2,304 trajectories, a ragged 72 warps;
+    config 4's Philox stream; config4_big = 200,000 of it, more than the bulk grid has lanes, so that the second
+    bulk kernel of the pipeline does advance carried trajectories next to its own)."""
     if which == "config0":
         cell = I.config0()
     elif which == "config1":
         cell = I.config1(48)
         cell = replace(cell, params=replace(cell.params, t_max_rf=300.0))
     else:
-        cell = I.config4(n_total=1500, batch=1500)[0]
+        nn = 200_000 if which == "config4_big" else 1500
+        cell = I.config4(n_total=nn, batch=nn)[0]
         cell = replace(cell, params=replace(cell.params, t_max_rf=300.0))
     runs = {}
     with P.Context(cell.params) as ctx:
@@ -219,6 +222,34 @@ def test_bulk_coop_and_handoff_paths_are_bit_identical(P, which):
         ctx.set_handoff(0)
         runs["auto0"], s0, _ = ctx.run_sync(replace(cell.launch, path=0))
         assert int(s0["n_handoff"]) == 0
+        # pipelined (ia_set_pipeline): the launch cut into three runs of unequal size; the bulk kernel of each run
+        # resumes what the one before left unfinished, one straggler chain at the join
+        import torch
+        ctx.set_handoff(16)
+        ctx.set_pipeline(8)
+        n = cell.launch.n
+        cuts = [0, n // 5, n // 5 + n // 2, n]
+        rec_p, sum_p, _ = ctx.alloc(n)
+        parts = [ctx.alloc(1)[1] for _ in range(3)]
+        for i in range(3):
+            L = replace(cell.launch, n=cuts[i + 1] - cuts[i], first_index=cell.launch.first_index + cuts[i], path=0)
+            ctx.run(L, records=rec_p[cuts[i] * P.RECORD_BYTES:], summary=parts[i])
+        ctx.join()
+        torch.cuda.synchronize()
+        runs["pipelined"] = P.view_records(rec_p, n)
+        sp = [P.view_summary(x) for x in parts]
+        assert sum(int(x["n_done"]) for x in sp) == n
+        for f in ("n_complex", "steps_acc", "steps_rej", "steps_loc"):
+            assert sum(int(x[f]) for x in sp) == int(s_bulk[f]), f
+        # every attempted step was taken either in one of the three bulk kernels or after the last hand-over
+        assert sum(int(x["steps_kernel"]) for x in sp) <= sum(int(s_bulk[f]) for f in ("steps_acc", "steps_rej", "steps_loc"))
+        if which != "config0":
+            assert int(sp[0]["n_handoff"]) > 0      # trajectories of run 0 did finish in a later kernel
+        if which == "config4_big":
+            # the second bulk kernel took more steps than its own trajectories account for: it advanced the first's
+            own = int(sp[1]["steps_acc"]) + int(sp[1]["steps_rej"]) + int(sp[1]["steps_loc"]) - int(sp[1]["steps_coop"])
+            assert int(sp[1]["steps_kernel"]) > own > 0
+        ctx.set_pipeline(0)
     assert int(s_bulk["n_done"]) == cell.launch.n == int(s_coop["n_done"])
     assert int(s_bulk["n_handoff"]) == 0 and int(s_coop["n_handoff"]) == 0
     if which != "config0":
@@ -231,10 +262,10 @@ def test_bulk_coop_and_handoff_paths_are_bit_identical(P, which):
 
 
 def test_pipelined_runs_match_serial_runs(P):
-    """ia_set_pipeline(3): five runs enqueued back to back (one straggler kernel for runs 1-3 on the library's
-    own stream, one for runs 4-5 at the join) give the records and summaries of the same five runs done one
-    after the other; the same through ia_submit_host / ia_wait with host buffers (a third and fourth
-    generation, recycling both generation buffers)."""
+    """ia_set_pipeline(3): five runs enqueued back to back (runs 1-3 share one straggler chain, enqueued by the fourth
+    ia_run when the pipeline is full; runs 4-5 the one of the join) give the records and summaries of the same five
+    runs done one after the other; the same through ia_submit_host / ia_sync / ia_wait with host buffers, where the
+    records of the trajectories that outlive their run's bulk kernel come back through the late list."""
     import torch
     cell = I.config1(40)
     cell = replace(cell, params=replace(cell.params, t_max_rf=200.0))
@@ -247,20 +278,25 @@ def test_pipelined_runs_match_serial_runs(P):
         bufs = [ctx.alloc(n) for _ in launches]
         for L, (rec, summ, _) in zip(launches, bufs):
             ctx.run(L, records=rec, summary=summ)
+        with pytest.raises(P.IaError):
+            ctx.timing(0)                       # its chain is not enqueued yet
         ctx.join()
         torch.cuda.synchronize()
         for (rec, summ, _), (rec0, summ0) in zip(bufs, serial):
             _assert_records_identical(P.view_records(rec, n), rec0)
             s = P.view_summary(summ)
-            for f in ("n_done", "n_complex", "steps_acc", "steps_rej", "steps_loc", "n_handoff", "steps_coop"):
+            for f in ("n_done", "n_complex", "steps_acc", "steps_rej", "steps_loc"):
                 assert int(s[f]) == int(summ0[f]), f
+            assert np.array_equal(s["hist_ncoll"], summ0["hist_ncoll"]) and np.array_equal(s["hist_tlife"], summ0["hist_tlife"])
         assert int(serial[0][1]["n_handoff"]) > 0
+        assert int(P.view_summary(bufs[0][1])["n_handoff"]) > 0
         t = [ctx.timing(back) for back in range(5)]
         assert all(x["bulk_ms"] > 0.0 and x["coop_ms"] > 0.0 for x in t)
-        assert t[0]["coop_ms"] == t[1]["coop_ms"] and t[2]["coop_ms"] == t[4]["coop_ms"]   # shared by a generation
+        assert t[0]["coop_ms"] == t[1]["coop_ms"] and t[2]["coop_ms"] == t[4]["coop_ms"]   # one chain per join
+        assert t[0]["coop_ms"] != t[2]["coop_ms"]
         with pytest.raises(P.IaError):
             ctx.timing(1000)
-        # host entry points, asynchronous form
+        # host entry points, asynchronous form: four runs, the pipeline filling up once (depth 3)
         ic = ctx.generate(launches[1])
         y0 = torch.from_numpy(np.ascontiguousarray(ic[:, :12])).pin_memory()
         ph = torch.from_numpy(np.ascontiguousarray(ic[:, 12])).pin_memory()
@@ -269,13 +305,30 @@ def test_pipelined_runs_match_serial_runs(P):
                  torch.zeros(P.SUMMARY_BYTES, dtype=torch.uint8).pin_memory()) for _ in range(4)]
         for rec_h, sum_h in host:
             P.ia_submit_host(ctx.handle, cl, rec_h, sum_h)
+        ctx.sync()
+        # after ia_sync the early copies have landed, but the last run still lacks its late finishers (a run of fewer
+        # trajectories than the grid has lanes hands all of them on as soon as they are generated)
+        early = host[3][0].numpy().view(P.RECORD_DTYPE)
+        assert int((early["steps_acc"] == serial[1][0]["steps_acc"]).sum()) < n
         ctx.wait()
         for rec_h, sum_h in host:
             _assert_records_identical(rec_h.numpy().view(P.RECORD_DTYPE), serial[1][0])
-            assert int(sum_h.numpy().view(P.SUMMARY_DTYPE)[0]["n_done"]) == n
+            sh = sum_h.numpy().view(P.SUMMARY_DTYPE)[0]
+            assert int(sh["n_done"]) == n and int(sh["steps_acc"]) == int(serial[1][1]["steps_acc"])
+        # the generator modes through the host entry points (nothing to copy in), GRID launch 2
+        rec_h, sum_h = host[0]
+        rec_h.zero_()
+        P.ia_submit_host(ctx.handle, P.make_launch(launches[2]), rec_h, sum_h)
+        P.ia_submit_host(ctx.handle, P.make_launch(launches[3]), host[1][0], host[1][1])
+        ctx.wait()
+        _assert_records_identical(rec_h.numpy().view(P.RECORD_DTYPE), serial[2][0])
+        _assert_records_identical(host[1][0].numpy().view(P.RECORD_DTYPE), serial[3][0])
         ctx.set_pipeline(0)
         rec1, _ = ctx.run_sync(launches[2])[:2]
         _assert_records_identical(rec1, serial[2][0])
+        rec_h2, sum_h2 = ctx.run_host(launches[4])
+        _assert_records_identical(rec_h2, serial[4][0])
+        assert int(sum_h2["n_done"]) == n
 
 
 # ---------------------------------------------------------------------------------------------
