@@ -86,8 +86,7 @@ typedef enum {
                            rf phase as phase_mode says                                              */
 } ia_ic_mode;
 
-/* Launches of the cooperative kernel per straggler phase: a chain of levels, each lasting twice as long
- * as the one before and re-packing what that one had left ten trajectories to a warp. */
+/* Most launches of the cooperative kernel at the end of a straggler chain (ia_set_chain). */
 #define IA_STRAGGLER_LEVELS 12
 
 /* Which kernels propagate a launch.  The bulk kernel runs one lane per trajectory; once the work
@@ -263,11 +262,14 @@ int ia_get_kernel_info(const ia_ctx *ctx, int kernel, int *warps_per_sm, int *n_
  * kernel with ten trajectories per warp does the work of ~18 bulk lanes). */
 int ia_set_handoff(ia_ctx *ctx, int lanes);
 
-/* The straggler chain: the cooperative kernel is launched `levels` times in a row
- * (1..IA_STRAGGLER_LEVELS, the default).  Level j = 0, 1, ... runs until its queue is empty and then for
- * budget << j further iterations per warp (default 8192, at least 64); what still runs then goes to the
- * next level, which packs it ten trajectories to a warp again.  The last level keeps everything.
- * levels = 1: one launch finishes all stragglers.  Applies to the straggler phases enqueued afterwards. */
+/* The straggler chain moves what a bulk kernel left unfinished into ever fewer warps, because
+ * the latency of a step falls with the number of warps that share an SM sub-partition: the bulk kernel over a
+ * full grid until at most 128 x #SM trajectories run, the bulk kernel with one warp per sub-partition until at
+ * most 40 x #SM run, then the cooperative kernel with one warp per sub-partition, `levels` times in a row
+ * (1..IA_STRAGGLER_LEVELS; default 1: one launch finishes everything).  With levels > 1, cooperative level
+ * j = 0, 1, ... runs until its queue is empty and then for budget << j further iterations per warp (default
+ * 8192, at least 64); what still runs then goes to the next level, which packs it ten trajectories to a warp
+ * again; the last level keeps everything.  Applies to the chains enqueued afterwards. */
 int ia_set_chain(ia_ctx *ctx, int levels, uint32_t budget);
 
 /* Device times of a run of this ctx, from CUDA events the library records around its kernels: the run's

@@ -29,25 +29,27 @@ struct IaKernelInfo {
 #define IA_COUNTER_RING 256 /* work counters of the runs that need no queue */
 #define IA_NSTAGE 3         /* device staging buffers of the host entry points */
 
-/* The straggler chain: the cooperative kernel is launched IA_STRAGGLER_LEVELS times in a
- * row.  Level j runs until its queue is empty and then for level_budget << j more iterations per warp; what
- * still runs then is passed on to level j+1, which packs it ten trajectories to a warp again, in the
- * lowest-numbered blocks.  The survivors -- the longest trajectories -- so end up in a few dense warps, each
- * with an SM sub-partition to itself, where the latency of a step is lowest, instead of in thousands of
- * thinned-out warps that share sub-partitions.  A level lasts twice as long as the one before, so a
- * trajectory of N steps passes ~log2(N / budget) hand-overs of 256 bytes.  The last level keeps everything. */
+/* The straggler chain.  What decides the latency of a step is how many warps share an SM
+ * sub-partition (measured, profiles/r02_latency_vs_occupancy.md: bulk layout 2.61 / 1.84 / 1.14 us per step at
+ * 3 / 2 / 1 warps, cooperative layout 1.01 us at 1 warp with a third of the trajectories per warp).  The chain
+ * therefore moves what is left into ever fewer warps, by COUNT: stage A = the bulk kernel over a full grid until
+ * at most 32 x 4 x #SM trajectories run; stage B = the bulk kernel with one warp per sub-partition until at most
+ * 10 x 4 x #SM run; stage C = the cooperative kernel, one warp per sub-partition, `levels` launches (the re-packing
+ * levels of ia_set_chain: level j passes on what still runs level_budget << j iterations after its queue ran dry;
+ * the last keeps everything; one level by default). */
 #define IA_BULK_BUDGET 4096u /* the bulk kernel: a warp hands over at the latest this long after the counter ran dry */
 
 /* Device words of the open pipeline cycle (all zeroed when a cycle starts):
  *   cnt[k], k = 0..IA_PIPE_MAX: trajectories handed INTO run k of the cycle (cnt[0] stays 0; run k counts what it
  *                               hands on in cnt[k+1]); cnt[n_open] is what the straggler chain starts from
  *   wc[k]:                      work counter of run k's bulk kernel
- *   chain[2j], chain[2j+1]:     level j >= 1 of the chain: trajectories queued for it, its work counter
- *                               (level 0 uses cnt[n_open] and chain[1])                                   */
+ *   chain[3j .. 3j+2]:          stage j of the chain: trajectories queued for it (stage 0 uses cnt[n_open]),
+ *                               its work counter, the trajectories it has finished                        */
 #define IA_W_CNT 0
 #define IA_W_WC (IA_W_CNT + IA_PIPE_MAX + 1)
 #define IA_W_CHAIN (IA_W_WC + IA_PIPE_MAX)
-#define IA_W_TOTAL (IA_W_CHAIN + 2 * IA_STRAGGLER_LEVELS + 2)
+#define IA_CHAIN_STAGES (2 + IA_STRAGGLER_LEVELS)
+#define IA_W_TOTAL (IA_W_CHAIN + 3 * IA_CHAIN_STAGES + 3)
 
 struct IaRunEvents {
     cudaEvent_t ev[2] = {nullptr, nullptr}; /* around the bulk kernel */
@@ -81,7 +83,7 @@ struct ia_ctx {
     size_t queue_cap = 0; /* hand-over entries one bulk kernel can produce: one per lane of a full grid */
     int handoff_lanes = 16;
     double w_harm = 0.0;                   /* |q_x| Omega / 2^(3/2): the ion's trap frequency in thermal runs */
-    int levels = IA_STRAGGLER_LEVELS;      /* launches of the straggler chain (ia_set_chain) */
+    int levels = 1;                        /* launches of the cooperative kernel at the end of the chain (ia_set_chain) */
     unsigned level_budget = 8192u;         /* iterations of its first level after the queue ran dry */
     int n_sm = 0;
     IaKernelInfo kinfo[2]; /* 0 bulk, 1 cooperative */
@@ -446,31 +448,38 @@ static int flush_open(ia_ctx *ctx, cudaStream_t st) {
     IaGen G0;
     std::memset(&G0, 0, sizeof(G0));
     IaOut O0 = {nullptr, nullptr, nullptr}; /* every queue entry carries the outputs of its own run */
-    /* what level 0 may find: every lane of a full bulk grid (a pipelined bulk kernel hands over all it holds),
-     * or the lanes the hand-over threshold lets through */
-    unsigned long long most = ctx->queue_cap;
-    if (ctx->depth == 0 && ctx->handoff_lanes < 32) most = ctx->queue_cap / 32ull * (unsigned long long)ctx->handoff_lanes;
     int qi = (ctx->n_open - 1) & 1; /* the queue the last bulk kernel wrote */
     unsigned long long *chain = ctx->words + IA_W_CHAIN;
+    const int sparse = ctx->n_sm * 4; /* one warp per SM sub-partition */
+    const int n_stages = 2 + ctx->levels;
     IaFlush &F = ctx->flush[ctx->flush_next % IA_FLUSH_RING];
     e = cudaEventRecord(F.ev[0], st);
-    for (int j = 0; j < ctx->levels && e == cudaSuccess; ++j) {
+    for (int j = 0; j < n_stages && e == cudaSuccess; ++j) {
         IaSched S5;
         std::memset(&S5, 0, sizeof(S5));
         sched_late(ctx, &S5);
         S5.q_in = ctx->q[qi];
-        S5.n_in = j == 0 ? ctx->words + IA_W_CNT + ctx->n_open : chain + 2 * j;
-        S5.counter = chain + 2 * j + 1;
-        if (j + 1 < ctx->levels) {
+        S5.n_in = j == 0 ? ctx->words + IA_W_CNT + ctx->n_open : chain + 3 * j;
+        S5.counter = chain + 3 * j + 1;
+        const bool last = j + 1 == n_stages;
+        if (!last) {
             S5.q_out = ctx->q[qi ^ 1];
-            S5.n_out = chain + 2 * (j + 1);
+            S5.n_out = chain + 3 * (j + 1);
             S5.handoff_lanes = 0;
-            const unsigned long long b = (unsigned long long)ctx->level_budget << j;
-            S5.budget = b > 0xffffffffull ? 0xffffffffu : (unsigned)b;
+            S5.budget = 0xffffffffu;
         }
-        const int blocks = grid_for(ctx, 1, most);
-        e = ia_launch_persistent(3, ctx->P, G0, O0, S5, blocks, st);
-        most = (unsigned long long)blocks * 10ull; /* what level j can pass on at most: all it holds */
+        if (j < 2) {
+            /* stages A, B: bulk layout, leaving by count */
+            S5.n_fin = chain + 3 * j + 2;
+            S5.run_floor = (unsigned long long)sparse * (j == 0 ? 32ull : 10ull);
+            e = ia_launch_persistent(1, ctx->P, G0, O0, S5, j == 0 ? grid_for(ctx, 0, ~0ull >> 8) : sparse, st);
+        } else {
+            if (!last) {
+                const unsigned long long b = (unsigned long long)ctx->level_budget << (j - 2);
+                S5.budget = b > 0xffffffffull ? 0xffffffffu : (unsigned)b;
+            }
+            e = ia_launch_persistent(3, ctx->P, G0, O0, S5, sparse, st);
+        }
         qi ^= 1;
     }
     if (e == cudaSuccess) e = cudaEventRecord(F.ev[1], st);

@@ -395,7 +395,16 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
         if (S.q_out != nullptr && wexh) {
             const unsigned am = __ballot_sync(IA_FULL, mode == MODE_RUN && L.leader); /* one bit per trajectory */
             const unsigned lm = __ballot_sync(IA_FULL, mode == MODE_LOC);
-            if (am != 0u && lm == 0u && (__popc(am) <= S.handoff_lanes || cnt >= S.budget)) {
+            /* a stage of the straggler chain also leaves when few of its trajectories are left altogether: the
+             * next stage runs them in fewer warps per SM sub-partition, i.e. at a lower latency per step */
+            bool few = false;
+            if (S.n_fin != nullptr) {
+                unsigned long long f = 0;
+                if (lane == 0) f = *(volatile unsigned long long *)S.n_fin;
+                f = __shfl_sync(IA_FULL, f, 0);
+                few = IA_N_IN - f <= S.run_floor;
+            }
+            if (am != 0u && lm == 0u && (__popc(am) <= S.handoff_lanes || cnt >= S.budget || few)) {
                 const int first = __ffs(am) - 1;
                 unsigned long long base = 0;
                 if ((int)lane == first) base = atomicAdd(S.n_out, (unsigned long long)__popc(am));
@@ -604,6 +613,7 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
                     if (SRC != IA_SRC_QUEUE && O.summary != nullptr)
                         atomicAdd((unsigned long long *)&O.summary->steps_kernel,
                                   (unsigned long long)(steps_acc + steps_rej + n_loc - steps_entry));
+                    if (S.n_fin != nullptr) atomicAdd(S.n_fin, 1ull);
                     if (out_sum != nullptr) {
                         ia_summary *Sm = out_sum;
                         atomicAdd((unsigned long long *)&Sm->n_done, 1ull);

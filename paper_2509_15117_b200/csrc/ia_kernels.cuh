@@ -62,6 +62,8 @@ struct IaSched {
     unsigned long long *n_out;       /* ... counting them here                                           */
     int handoff_lanes;               /* ... once the counter is empty and <= this many trajectories of a warp run */
     unsigned budget;                 /* ... or once it has run this many iterations since the counter ran dry */
+    unsigned long long *n_fin;       /* non-NULL: counts the trajectories this kernel finishes; a warp hands over  */
+    unsigned long long run_floor;    /* ... also once at most this many of the n_in it resumed are still running   */
     unsigned long long warn;
     IaLate *late;                    /* list of finished trajectories whose records live on the host ...  */
     unsigned long long *n_late;      /* ... its length ...                                                */
