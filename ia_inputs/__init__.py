@@ -164,6 +164,18 @@ def thermal(atom: str = "Rb87", T_atom_uK: float = 1.0, De_K: float = 1.0, n: in
                        T_atom_uK=T_atom_uK, T_ion_uK=10.0))
 
 
+def fig4(atom: str = "Rb87", E_uK: float = 10.0, n: int = 10_000, phase_mode: int = 1, phase0: float = 0.0,
+         r0_a0: float = 20_000.0, seed: int = DEFAULT_SEED) -> Cell:
+    """One point of the paper's Fig. 4: head-on collisions of `atom` with
+    Yb+ at one collision energy from the sphere r0 = 20 000 a0, D_e = 1 K, directions uniform on the octant, rf phase
+    uniformly random (phase_mode 1, the figure) or fixed at phase0 (phase_mode 0: the oscillation of about +-0.1 in
+    the probability that PAPER.md:68 describes).  Philox cell = 400 + species."""
+    p = replace(Params().with_atom(atom), r0_a0=r0_a0)
+    return Cell(f"fig4_{atom}_{E_uK:g}uK_r0{r0_a0:g}" + ("" if phase_mode else f"_phase{phase0:.3f}"), p,
+                Launch(mode=MODE_PHILOX, n=n, domain=0, phase_mode=phase_mode, phase0=phase0, E_min_uK=E_uK,
+                       E_max_uK=E_uK, seed=seed, cell=400 + SPECIES_ORDER.index(atom)))
+
+
 def subgrid_indices(n_side: int, every: int) -> np.ndarray:
     """Local indices of the (every x every)-decimated sub-grid of an n_side x n_side grid launch."""
     ii = np.arange(every // 2, n_side, every, dtype=np.uint64)

@@ -359,9 +359,21 @@ def test_config0_adaptive_parity_full(P):
     assert np.all(ref["n_coll"] == 1) and np.all(ref["status"] == 0)             # all regular
     assert np.array_equal(rec["n_coll"], ref["n_coll"]) and np.array_equal(rec["n_tp"], ref["n_tp"])
     same, e_t, e_dir, e_v, e_k = _compare_regular(rec, ref, "config0 (same ICs)")
-    assert same.mean() >= 0.99
+    # SURVEY A15 expects <~ 1e-4 flipped accept/reject decisions; measured on this grid: none
+    assert (~same).sum() <= 2, f"{(~same).sum()} of 1024 step sequences differ"
     assert e_t[same].max() <= 1e-8 and e_dir[same].max() <= 1e-8 and e_v[same].max() <= 1e-8
-    assert np.median(e_k[same]) <= 1e-8 and e_k[same].max() <= 3e-7
+    # ke_ion carries the micromotion phase Omega t of the exit time: a relative 1e-9 in t_dwell (inside the bar above)
+    # is 2 pi (t_dwell/T_rf) 1e-9 = 3e-8 of the oscillation.  Reading R19: the floor measured oracle against oracle
+    # (tests/test_oracle_pins2.py: the same source with fused multiply-adds) is median 1.2e-9 / maximum 4e-8 on this
+    # grid; the CUDA path is held to 2.5 times that (measured: 2.3e-9 / 9.7e-8), and its ke_ion error must be the
+    # phase error of its t_dwell error, not something else:
+    assert np.median(e_k[same]) <= 3e-9 and np.quantile(e_k[same], 0.99) <= 5e-8 and e_k[same].max() <= 1e-7
+    T_rf = 2.067068666759e10
+    phase_err = 2.0 * np.pi * np.abs(rec["t_dwell"] - ref["t_dwell"]) / T_rf
+    ratio = e_k[same] / np.maximum(phase_err[same], 1e-12)
+    print("   ke_ion error / micromotion phase error of the exit time, quantiles 50/90/100 %: "
+          + "/".join(f"{x:.2f}" for x in np.quantile(ratio, [0.5, 0.9, 1.0])))
+    assert np.median(ratio) <= 5.0
     # flipped decisions: still the same trajectory at truncation level (R15)
     if (~same).any():
         assert e_t[~same].max() < 1e-3 and e_k[~same].max() < 5e-2
@@ -478,13 +490,20 @@ def test_config1_full_grid_in_the_bench_configuration(P):
     assert np.all(rec["n_coll"][rec["status"] == 0] >= 1)                      # head-on: every escape bounced once
 
 
-@pytest.mark.parametrize("which,ci", [("config2", 18), ("config2", 2), ("config3", 7), ("config4", 0)])
+@pytest.mark.parametrize("which,ci", [("config2", 18), ("config2", 2), ("config3", 7), ("config4", 0),
+                                      ("config3", 0), ("config3", 4), ("config3", 10), ("config3", 14)])
 def test_philox_cells_ensemble(P, which, ci):
     """First 2^12 Philox indices of one cell of configs 2-4: Rb 30 uK (near the threshold),
-    Li 10 uK (no complexes), a D_e = 1 K / q = 0.2 cell of config 3, and config 4's log-uniform stream."""
+    Li 10 uK (no complexes), a D_e = 1 K / q = 0.2 cell of config 3, config 4's log-uniform stream, and the corners
+    q = 0.05 and q = 0.4 of config 3's D_e = 0.1 K and D_e = 10 K rows (the latter: 2^11 indices and t_max cut to
+    300 T_rf so that the oracle finishes -- a complex still bound then counts as one on both sides)."""
     n = 4096
     cell = {"config2": I.config2, "config3": I.config3}.get(which, None)
+    if which == "config3" and ci >= 10:
+        n = 2048
     cell = cell(n_per_cell=n)[ci] if cell else I.config4(n_total=n, batch=n)[0]
+    if which == "config3" and ci >= 10:
+        cell = replace(cell, params=replace(cell.params, t_max_rf=300.0))
     with P.Context(cell.params) as ctx:
         rec, summ, _ = ctx.run_sync(cell.launch)
     ref = O.run_generated(cell.params, cell.launch, nthreads=NTHREADS)
@@ -631,3 +650,120 @@ def test_deep_well_cell_ensemble(P):
     assert reg.sum() > 500 and same.mean() >= 0.95
     assert np.median(e_t[same]) <= 1e-5 and np.median(e_dir[same]) <= 1e-5
     assert int(summ["n_done"]) == 2048 and rec["n_loc"].max() < 60
+
+
+# ---------------------------------------------------------------------------------------------
+# Fig. 4's start radius r0 = 20 000 a0 and the fixed-phase runs
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("variant", [0, 1])
+def test_r0_20000_one_step_map(P, variant):
+    """The one-step map (R12) on states sampled along oracle trajectories that start at r0 = 20 000 a0: four times
+    the free flight of configs 0-4, i.e. mostly micromotion-limited far-field steps at |r_a| up to 2e4 a0."""
+    cell = I.fig4("Rb87", 10.0, n=64)
+    tf, ph, y, h = _sampled_states(cell, n_traj=5, seed=9)
+    assert np.linalg.norm(y[:, 3:6], axis=1).max() > 1.5e4 and np.linalg.norm(y[:, 3:6] - y[:, 0:3], axis=1).min() < 80.0
+    ref = np.stack([O.step(cell.params, tf[k], ph[k], y[k], h[k])[0] for k in range(len(y))])
+    with P.Context(cell.params) as ctx:
+        got, _ = ctx.step_map(tf, ph, y, h, variant=variant)
+    rel = block_rel(got, ref, 1e-3 * np.linalg.norm(y[:, 9:12], axis=1).max())
+    print(f"\none-step map r0 = 20 000 a0 variant={variant}: n={len(y)} max block rel diff {rel.max(axis=0)}")
+    assert rel.max() <= 1e-12
+
+
+def test_r0_20000_ensemble(P):
+    """Fig. 4's setting: Yb+ + 87Rb head-on from r0 = 20 000 a0 at 10 uK, random rf phase, 4 096
+    trajectories against the oracle (t_max cut to 2 000 T_rf on both sides to bound the oracle's run): ensemble
+    statistics within the 99 % intervals, and the single-bounce trajectories one by one."""
+    cell = I.fig4("Rb87", 10.0, n=4096)
+    cell = replace(cell, params=replace(cell.params, t_max_rf=2000.0))
+    with P.Context(cell.params) as ctx:
+        rec, summ, _ = ctx.run_sync(cell.launch)
+    ref = O.run_generated(cell.params, cell.launch, nthreads=NTHREADS)
+    ok, detail = _ensemble_checks(rec, ref, cell.name)
+    assert ok, detail
+    assert int(summ["warn"]) == 0           # 10 |V(r0)| < E holds easily at this radius (PAPER.md:28)
+    reg = (ref["n_coll"] == 1) & (rec["n_coll"] == 1) & (ref["status"] == 0) & (rec["status"] == 0)
+    same, e_t, e_dir, e_v, e_k = _compare_regular(rec[reg], ref[reg], "r0 = 20 000 a0 regular region")
+    # Reading R20: over a free flight of 180 rf periods (10^4 micromotion-limited steps) the step-size sequence is itself a
+    # chaotic function of round-off -- a relative 1e-9 in one error estimate doubles from step to step until an
+    # accept/reject decision flips (followed attempt by attempt with the oracle's and the device's one-step maps: the
+    # device's controller reproduces its own record exactly, and no single decision is close to the threshold).
+    # Measured: 0 of 587 sequences differ at r0 = 5 000 a0, 43 of 554 at 10 000, 236 of 555 at 20 000.  A trajectory
+    # with a different sequence is the same solution at truncation level (R15): held to 1e-3 / 5e-2 below.
+    assert reg.sum() > 500 and 0.3 <= same.mean()
+    assert np.median(e_t[same]) <= 1e-8 and np.median(e_dir[same]) <= 1e-8
+    assert e_t.max() < 1e-3 and e_dir.max() < 1e-2 and np.quantile(e_k, 0.99) < 5e-2
+    steps = rec["steps_acc"].astype(np.int64) + rec["steps_rej"]
+    print(f"   steps per trajectory: median {np.median(steps):.0f} mean {steps.mean():.0f}")
+
+
+def test_fixed_phase_oscillation(P):
+    """with the initial rf phase fixed instead of random, the complex-formation probability at a given
+    energy moves by about +-0.1 with the phase.  Eight fixed phases at Rb 10 uK from r0 = 20 000 a0: the CUDA path
+    against the oracle phase by phase (1 024 trajectories each, 99 % interval of the difference), then the spread over
+    the phases at 2^15 trajectories per phase on the GPU alone, against the phase-averaged (random-phase) value."""
+    phases = [2.0 * np.pi * k / 8 for k in range(8)]
+    base = I.fig4("Rb87", 10.0, n=1024, phase_mode=0)
+    params = replace(base.params, t_max_rf=500.0)
+    p_gpu = []
+    with P.Context(params) as ctx:
+        for ph in phases:
+            L = replace(base.launch, phase0=ph)
+            rec, _, _ = ctx.run_sync(L)
+            ref = O.run_generated(params, L, nthreads=NTHREADS)
+            k_g, k_o = int((rec["n_coll"] >= 2).sum()), int((ref["n_coll"] >= 2).sum())
+            ok, d, half = S.two_proportion_ok(k_g, L.n, k_o, L.n)
+            assert ok, (ph, k_g, k_o)
+            big = replace(L, n=1 << 15)
+            _, sb, _ = ctx.run_sync(big)
+            p_gpu.append(int(sb["n_complex"]) / big.n)
+        _, sr, _ = ctx.run_sync(replace(base.launch, n=1 << 17, phase_mode=1))
+    p_rand = int(sr["n_complex"]) / (1 << 17)
+    p_gpu = np.array(p_gpu)
+    print(f"\nfixed phase, Rb 10 uK, r0 = 20 000 a0: P(complex) per phase {np.round(p_gpu, 4)}; "
+          f"spread +-{0.5 * (p_gpu.max() - p_gpu.min()):.3f} around {p_gpu.mean():.4f}; random phase {p_rand:.4f}")
+    se = np.sqrt(0.25 / (1 << 15))
+    assert p_gpu.max() - p_gpu.min() > 8 * se                 # the probability does depend on the phase ...
+    assert 0.02 < 0.5 * (p_gpu.max() - p_gpu.min()) < 0.3     # ... by the order of magnitude the paper states
+    assert abs(p_gpu.mean() - p_rand) < 5 * se                # and the random-phase run is its average
+
+
+# ---------------------------------------------------------------------------------------------
+# SURVEY.md section 8(f) item 4: the (theta, phi) images of Fig. 1 from GPU records (PAPER.md:24)
+# ---------------------------------------------------------------------------------------------
+def test_maps_from_gpu_records(P):
+    """64 x 64 octant map of config 1 (Fig. 1): scattering angle arccos(v_i.v_f/(v_i v_f)), log10 of the
+    number of bounces and the momentum transfer clipped at 0.015 a.u., built by observables.maps from the GPU's
+    records and generated initial conditions, against the same images built from the oracle's outcomes and the
+    oracle's own generator.  Pixel by pixel on the regular region (one bounce, identical step sequences); as counts
+    where the trajectories are chaotic (R14)."""
+    from paper_2509_15117_b200 import observables as Ob
+    cell = I.config1(64)
+    with P.Context(cell.params) as ctx:
+        rec, summ, ic = ctx.run_sync(cell.launch, want_ic=True)
+        m_a = ctx.derived["m_a"]
+    ref = O.run_generated(cell.params, cell.launch, nthreads=NTHREADS)
+    y0, ph, _ = O.generate(cell.params, cell.launch, np.arange(cell.launch.n, dtype=np.uint64))
+    ic_o = np.concatenate([y0, ph[:, None], np.zeros((len(ph), 1))], axis=1)
+    g = Ob.maps(rec, ic, m_a, 64, 64)
+    o = Ob.maps(ref, ic_o, O.derive(cell.params)["m_a"], 64, 64)
+    for k in g:
+        assert g[k].shape == (64, 64)
+    same = ((rec["steps_acc"] == ref["steps_acc"]) & (rec["steps_rej"] == ref["steps_rej"])).reshape(64, 64)
+    reg = same & ~g["complex"] & ~o["complex"]
+    assert reg.sum() > 1500
+    d_chi = np.abs(g["scattering_angle"] - o["scattering_angle"])[reg]
+    d_q = (np.abs(g["momentum_transfer_clipped"] - o["momentum_transfer_clipped"]) / o["momentum_transfer_clipped"])[reg]
+    agree = (g["complex"] == o["complex"]).mean()
+    print(f"\nFig. 1 maps 64x64: regular pixels {reg.sum()}, max |d chi| {d_chi.max():.2e} rad, max rel d q {d_q.max():.2e}; "
+          f"complex/regular classification agrees on {agree:.4f} of the pixels; complexes gpu {g['complex'].sum()} "
+          f"oracle {o['complex'].sum()}; clipped pixels gpu {(g['momentum_transfer_clipped'] >= Ob.Q_CLIP_AU).sum()} "
+          f"oracle {(o['momentum_transfer_clipped'] >= Ob.Q_CLIP_AU).sum()}")
+    assert np.array_equal(g["log10_bounces"][reg], o["log10_bounces"][reg])
+    assert d_chi.max() < 1e-5 and d_q.max() < 1e-5
+    assert agree > 0.99
+    # the head-on single-bounce atom comes back: scattering angle near pi (PAPER.md:30 "scatters backwards")
+    assert np.median(g["scattering_angle"][reg]) > 2.5
+    assert S.two_proportion_ok(int(g["complex"].sum()), 4096, int(o["complex"].sum()), 4096)[0]
+    # the phi = pi/4 saddle line (q_x = -q_y) is complex-dominated (PAPER.md:30-36): the two columns next to it
+    assert g["complex"][:, 31:33].mean() > g["complex"].mean()
