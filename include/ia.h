@@ -286,6 +286,14 @@ int ia_get_last_timing(ia_ctx *ctx, double *bulk_ms, double *coop_ms);
  * tflops = 2 * DFMA/s / 1e12; elapsed_ms = CUDA-event time of the timed launch. */
 int ia_fp64_peak(int cuda_device, double target_ms, double *tflops, double *elapsed_ms);
 
+/* Debugging aid (compute-sanitizer is not available on every machine): every device buffer a ctx owns -- hand-over
+ * queues, counters, summaries and records staged for the host entry points, the late-record list -- is allocated
+ * with 4 KiB guard zones of a known byte pattern on either side, and the kernels refuse to write a queue or list
+ * entry beyond the capacity they were given, setting a fault word instead.  ia_debug_check blocks until the ctx's
+ * work in flight has finished, then verifies every guard zone, the fault word and the device-side counts
+ * (IA_ECUDA / IA_EINVAL with the finding in ia_last_error). */
+int ia_debug_check(ia_ctx *ctx);
+
 int ia_destroy(ia_ctx *ctx);
 const char *ia_strerror(int code);
 const char *ia_last_error(const ia_ctx *ctx); /* "" if none; valid until the next call on ctx */

@@ -32,7 +32,7 @@ IA_STRAGGLER_LEVELS = 12
 # every symbol include/ia.h declares (tests/test_cabi.py checks the library exports each of them)
 EXPORTS = ("ia_create", "ia_run", "ia_run_host", "ia_generate", "ia_step_map", "ia_trace", "ia_get_derived",
            "ia_get_kernel_info", "ia_set_handoff", "ia_set_chain", "ia_get_last_timing", "ia_get_timing", "ia_set_pipeline", "ia_join",
-           "ia_submit_host", "ia_sync", "ia_wait", "ia_fp64_peak", "ia_destroy", "ia_strerror", "ia_last_error")
+           "ia_submit_host", "ia_sync", "ia_wait", "ia_debug_check", "ia_fp64_peak", "ia_destroy", "ia_strerror", "ia_last_error")
 
 
 class IaError(RuntimeError):
@@ -117,6 +117,7 @@ def load() -> C.CDLL:
     L.ia_submit_host.argtypes = [vp, C.POINTER(ia_launch), C.POINTER(ia_outputs)]
     L.ia_wait.argtypes = [vp]
     L.ia_sync.argtypes = [vp]
+    L.ia_debug_check.argtypes = [vp]
     L.ia_fp64_peak.argtypes = [C.c_int, C.c_double, dp, dp]
     L.ia_destroy.argtypes = [vp]
     L.ia_strerror.argtypes = [C.c_int]
@@ -293,6 +294,11 @@ def ia_sync(handle) -> None:
     _check(load().ia_sync(handle), handle)
 
 
+def ia_debug_check(handle) -> None:
+    """Verifies the guard zones around every ctx-owned device buffer and the kernels' fault word; raises on a finding."""
+    _check(load().ia_debug_check(handle), handle)
+
+
 def ia_fp64_peak(device: int = 0, target_ms: float = 200.0) -> dict:
     """DFMA peak microbenchmark: {'tflops': 2*DFMA/s/1e12, 'elapsed_ms': ...}."""
     t, ms = C.c_double(), C.c_double()
@@ -363,6 +369,9 @@ class Context:
 
     def sync(self) -> None:
         ia_sync(self.handle)
+
+    def debug_check(self) -> None:
+        ia_debug_check(self.handle)
 
     def alloc(self, n: int, ic_dump: bool = False):
         """(records uint8[n*64], summary uint8[1024] zeroed, ic_dump float64[n,14] or None) on the device."""

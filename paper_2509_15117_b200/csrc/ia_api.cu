@@ -7,6 +7,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <vector>
 
 #include "ia_kernels.cuh"
 
@@ -50,6 +51,8 @@ struct IaKernelInfo {
 #define IA_W_CHAIN (IA_W_WC + IA_PIPE_MAX)
 #define IA_CHAIN_STAGES (2 + IA_STRAGGLER_LEVELS)
 #define IA_W_TOTAL (IA_W_CHAIN + 3 * IA_CHAIN_STAGES + 3)
+#define IA_GUARD 4096       /* bytes of guard zone before and after every ctx-owned device buffer (ia_debug_check) */
+#define IA_GUARD_BYTE 0xA5
 
 struct IaRunEvents {
     cudaEvent_t ev[2] = {nullptr, nullptr}; /* around the bulk kernel */
@@ -59,6 +62,11 @@ struct IaRunEvents {
 struct IaFlush {
     cudaEvent_t ev[2] = {nullptr, nullptr}; /* around the chain */
     long long id = -1;
+};
+
+struct IaGuarded {
+    char *base = nullptr; /* what cudaMalloc returned */
+    size_t bytes = 0;     /* payload size */
 };
 
 struct IaStage {
@@ -106,10 +114,40 @@ struct ia_ctx {
     IaPending pending[IA_PIPE_MAX];
     int n_pending = 0;
     IaLate *late_dev = nullptr, *late_host = nullptr; /* records of late finishers of pipelined host runs */
-    unsigned long long *n_late = nullptr;             /* device counter */
+    unsigned long long *n_late = nullptr;             /* device counter; n_late[1] = the fault word of IaSched */
     unsigned long long late_cap = 0;
+    std::vector<IaGuarded> owned; /* every device buffer of the ctx, with its guard zones */
     std::string err;
 };
+
+/* device buffer with IA_GUARD bytes of a known pattern on either side (ia_debug_check verifies them) */
+static cudaError_t guarded_malloc(ia_ctx *c, void **out, size_t bytes) {
+    char *base = nullptr;
+    const size_t pay = (bytes + 255) & ~(size_t)255;
+    cudaError_t e = cudaMalloc(&base, pay + 2 * IA_GUARD);
+    if (e != cudaSuccess) return e;
+    e = cudaMemset(base, IA_GUARD_BYTE, IA_GUARD);
+    if (e == cudaSuccess) e = cudaMemset(base + IA_GUARD + pay, IA_GUARD_BYTE, IA_GUARD);
+    if (e != cudaSuccess) {
+        cudaFree(base);
+        return e;
+    }
+    IaGuarded g;
+    g.base = base;
+    g.bytes = pay;
+    c->owned.push_back(g);
+    *out = base + IA_GUARD;
+    return cudaSuccess;
+}
+static void guarded_free(ia_ctx *c, void *p) {
+    if (!p) return;
+    for (size_t k = 0; k < c->owned.size(); ++k)
+        if (c->owned[k].base + IA_GUARD == (char *)p) {
+            cudaFree(c->owned[k].base);
+            c->owned.erase(c->owned.begin() + k);
+            return;
+        }
+}
 
 static int fail_cuda(ia_ctx *c, const char *what, cudaError_t e) {
     if (c) c->err = std::string(what) + ": " + cudaGetErrorString(e);
@@ -213,19 +251,19 @@ int ia_create(ia_ctx **out, const ia_species *sp, const ia_trap *tr, double De_K
 
     c->n_sm = prop.multiProcessorCount;
     cudaError_t e = cudaSetDevice(cuda_device);
-    if (e == cudaSuccess) e = cudaMalloc(&c->counters, IA_COUNTER_RING * 4 * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = guarded_malloc(c, (void **)&c->counters, IA_COUNTER_RING * 4 * sizeof(unsigned long long));
     for (int k = 0; k < 2 && e == cudaSuccess; ++k)
         e = ia_persistent_info(k == 0 ? 1 : 3, &c->kinfo[k].blocks_per_sm, &c->kinfo[k].threads_per_block,
                                &c->kinfo[k].regs, &c->kinfo[k].local_bytes);
     if (e == cudaSuccess) {
         /* one entry per lane of a full bulk grid (a full cooperative grid holds fewer) */
         c->queue_cap = (size_t)c->n_sm * c->kinfo[0].blocks_per_sm * c->kinfo[0].threads_per_block;
-        for (int j = 0; j < 2 && e == cudaSuccess; ++j) e = cudaMalloc(&c->q[j], c->queue_cap * sizeof(IaHand));
+        for (int j = 0; j < 2 && e == cudaSuccess; ++j) e = guarded_malloc(c, (void **)&c->q[j], c->queue_cap * sizeof(IaHand));
     }
-    if (e == cudaSuccess) e = cudaMalloc(&c->words, IA_W_TOTAL * sizeof(unsigned long long));
-    if (e == cudaSuccess) e = cudaMalloc(&c->n_late, sizeof(unsigned long long));
-    if (e == cudaSuccess) e = cudaMemset(c->n_late, 0, sizeof(unsigned long long));
-    if (e == cudaSuccess) e = cudaMalloc(&c->sum_stage, IA_PIPE_MAX * sizeof(ia_summary));
+    if (e == cudaSuccess) e = guarded_malloc(c, (void **)&c->words, IA_W_TOTAL * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = guarded_malloc(c, (void **)&c->n_late, 2 * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMemset(c->n_late, 0, 2 * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = guarded_malloc(c, (void **)&c->sum_stage, IA_PIPE_MAX * sizeof(ia_summary));
     for (int k = 0; k < IA_RUN_RING && e == cudaSuccess; ++k)
         for (int j = 0; j < 2 && e == cudaSuccess; ++j) e = cudaEventCreate(&c->run[k].ev[j]);
     for (int k = 0; k < IA_FLUSH_RING && e == cudaSuccess; ++k)
@@ -252,17 +290,11 @@ int ia_destroy(ia_ctx *ctx) {
     if (ctx->ev_last && ctx->ev_last_valid) cudaEventSynchronize(ctx->ev_last);
     if (ctx->host_stream) cudaStreamSynchronize(ctx->host_stream);
     if (ctx->copy_stream) cudaStreamSynchronize(ctx->copy_stream);
-    for (int j = 0; j < 2; ++j)
-        if (ctx->q[j]) cudaFree(ctx->q[j]);
-    if (ctx->words) cudaFree(ctx->words);
-    if (ctx->n_late) cudaFree(ctx->n_late);
-    if (ctx->sum_stage) cudaFree(ctx->sum_stage);
-    if (ctx->late_dev) cudaFree(ctx->late_dev);
+    for (size_t k = 0; k < ctx->owned.size(); ++k) cudaFree(ctx->owned[k].base); /* queues, words, staging, ... */
+    ctx->owned.clear();
     if (ctx->late_host) cudaFreeHost(ctx->late_host);
-    for (int k = 0; k < IA_NSTAGE; ++k) {
-        if (ctx->stage[k].buf) cudaFree(ctx->stage[k].buf);
+    for (int k = 0; k < IA_NSTAGE; ++k)
         if (ctx->stage[k].ev_free) cudaEventDestroy(ctx->stage[k].ev_free);
-    }
     for (int k = 0; k < IA_FLUSH_RING; ++k)
         for (int j = 0; j < 2; ++j)
             if (ctx->flush[k].ev[j]) cudaEventDestroy(ctx->flush[k].ev[j]);
@@ -272,7 +304,6 @@ int ia_destroy(ia_ctx *ctx) {
     if (ctx->ev_last) cudaEventDestroy(ctx->ev_last);
     if (ctx->host_stream) cudaStreamDestroy(ctx->host_stream);
     if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
-    if (ctx->counters) cudaFree(ctx->counters);
     delete ctx;
     return IA_OK;
 }
@@ -424,6 +455,8 @@ static int grid_for(const ia_ctx *ctx, int k, unsigned long long n) {
 
 /* what every persistent kernel of the ctx is told about the late list (records wanted in host arrays) */
 static void sched_late(const ia_ctx *ctx, IaSched *S) {
+    S->q_cap = ctx->queue_cap;
+    S->fault = ctx->n_late + 1;
     S->late = ctx->late_dev;
     S->n_late = ctx->n_late;
     S->late_cap = ctx->late_dev ? ctx->late_cap : 0ull;
@@ -600,10 +633,10 @@ static int submit_host_impl(ia_ctx *ctx, const ia_launch *launch, const ia_outpu
     if (piped && host_out->records && !ctx->late_dev) {
         /* late list: at most one entry per lane of a bulk grid and run */
         const unsigned long long cap = (unsigned long long)ctx->queue_cap * IA_PIPE_MAX;
-        e = cudaMalloc(&ctx->late_dev, cap * sizeof(IaLate));
+        e = guarded_malloc(ctx, (void **)&ctx->late_dev, cap * sizeof(IaLate));
         if (e == cudaSuccess) e = cudaMallocHost(&ctx->late_host, cap * sizeof(IaLate));
         if (e != cudaSuccess) {
-            if (ctx->late_dev) cudaFree(ctx->late_dev);
+            guarded_free(ctx, ctx->late_dev);
             ctx->late_dev = nullptr;
             ctx->err = "late-record list allocation failed";
             return IA_ENOMEM;
@@ -619,10 +652,10 @@ static int submit_host_impl(ia_ctx *ctx, const ia_launch *launch, const ia_outpu
     if (total > T.bytes) {
         if (T.used) e = cudaEventSynchronize(T.ev_free); /* whatever still reads the old buffer finishes first */
         if (e != cudaSuccess) return fail_cuda(ctx, "synchronise before staging reallocation", e);
-        if (T.buf) cudaFree(T.buf);
+        guarded_free(ctx, T.buf);
         T.buf = nullptr;
         T.bytes = 0;
-        e = cudaMalloc(&T.buf, total);
+        e = guarded_malloc(ctx, (void **)&T.buf, total);
         if (e != cudaSuccess) {
             ctx->err = "device staging allocation failed";
             return IA_ENOMEM;
@@ -760,6 +793,41 @@ int ia_run_host(ia_ctx *ctx, const ia_launch *launch, const ia_outputs *host_out
     rc = wait_impl(ctx);
     if (rc == IA_OK) ctx->err = warn_text;
     return rc;
+}
+
+int ia_debug_check(ia_ctx *ctx) {
+    if (!ctx) return IA_EINVAL;
+    cudaError_t e = cudaSetDevice(ctx->device);
+    if (e == cudaSuccess && ctx->ev_last_valid) e = cudaEventSynchronize(ctx->ev_last);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->host_stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->copy_stream);
+    std::vector<unsigned char> g(2 * IA_GUARD);
+    for (size_t k = 0; k < ctx->owned.size() && e == cudaSuccess; ++k) {
+        const IaGuarded &G = ctx->owned[k];
+        e = cudaMemcpy(g.data(), G.base, IA_GUARD, cudaMemcpyDeviceToHost);
+        if (e == cudaSuccess) e = cudaMemcpy(g.data() + IA_GUARD, G.base + IA_GUARD + G.bytes, IA_GUARD, cudaMemcpyDeviceToHost);
+        for (size_t j = 0; j < g.size() && e == cudaSuccess; ++j)
+            if (g[j] != IA_GUARD_BYTE) {
+                char msg[160];
+                std::snprintf(msg, sizeof(msg), "ia_debug_check: guard zone of ctx buffer %zu (%zu bytes) overwritten at offset %s%zu",
+                              k, G.bytes, j < IA_GUARD ? "-" : "+", j < IA_GUARD ? IA_GUARD - j : j - IA_GUARD);
+                ctx->err = msg;
+                return IA_ECUDA;
+            }
+    }
+    unsigned long long w[2] = {0, 0};
+    std::vector<unsigned long long> words(IA_W_TOTAL);
+    if (e == cudaSuccess) e = cudaMemcpy(w, ctx->n_late, sizeof(w), cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess) e = cudaMemcpy(words.data(), ctx->words, IA_W_TOTAL * sizeof(unsigned long long), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return fail_cuda(ctx, "ia_debug_check", e);
+    if (w[1] != 0) {
+        ctx->err = (w[1] & 1) ? "ia_debug_check: a hand-over queue overflowed" : "ia_debug_check: the late-record list overflowed";
+        return IA_ECUDA;
+    }
+    if (ctx->late_dev && w[0] > ctx->late_cap) return fail_inval(ctx, "ia_debug_check: late-record count beyond capacity");
+    for (int k = 0; k <= IA_PIPE_MAX; ++k)
+        if (words[IA_W_CNT + k] > ctx->queue_cap) return fail_inval(ctx, "ia_debug_check: hand-over count beyond the queue capacity");
+    return IA_OK;
 }
 
 int ia_generate(ia_ctx *ctx, const ia_launch *launch, double *ic_dump, void *cuda_stream) {

@@ -61,9 +61,52 @@ struct IaIC {
     double phase, E_au;
 };
 
+/* THERMAL runs (reading R18) draw fourteen numbers per trajectory from seven Philox blocks; block b
+ * is one task: b = 0 -> (u1, u2), the direction of the atom's position; b = 1 -> (u3, u4), the rf phase;
+ * b = 2..6 -> a Box-Muller pair
+ * (z_2k, z_2k+1) = sqrt(-2 ln u_a) (cos 2 pi u_b, sin 2 pi u_b), k = b - 2.  The bulk kernel spreads the tasks of
+ * the lanes that start a trajectory over the whole warp (seven lanes work for one idle lane instead of the idle lane
+ * working seven times as long while 31 wait); ia_generate_ic runs them one after the other.  Same function, same
+ * inputs: the two give identical initial conditions. */
+__device__ __forceinline__ void ia_thermal_task(const IaGen &G, unsigned long long gi, unsigned b, double &a0, double &a1) {
+    unsigned w[4];
+    ia_philox((unsigned)gi, (unsigned)(gi >> 32), G.cell, b, (unsigned)G.seed, (unsigned)(G.seed >> 32), w);
+    const double ua = ia_u53(w[0], w[1]), ub = ia_u53(w[2], w[3]);
+    if (b < 2u) {
+        a0 = ua;
+        a1 = ub;
+    } else {
+        const double R = sqrt(-2.0 * log(ua));
+        double sb, cb;
+        sincospi(2.0 * ub, &sb, &cb);
+        a0 = R * cb;
+        a1 = R * sb;
+    }
+}
+
+/* the thermal initial condition from its fourteen numbers t[2b], t[2b+1] (see ia_thermal_task) */
+__device__ __forceinline__ void ia_thermal_assemble(const IaParams &P, const IaGen &G, const double *t, IaIC *ic) {
+    const double ct = 2.0 * t[0] - 1.0;
+    const double st = sqrt(1.0 - ct * ct);
+    double sp, cp;
+    sincospi(2.0 * t[1], &sp, &cp);
+    const double *z = t + 4;
+    const double n0 = st * cp, n1 = st * sp, n2 = ct;
+    double va0 = G.sig_v_atom * z[6], va1 = G.sig_v_atom * z[7], va2 = G.sig_v_atom * z[8];
+    const double vr = va0 * n0 + va1 * n1 + va2 * n2;
+    const double sign = (vr > 0.0) ? -1.0 : 1.0;
+    ic->E_au = 0.5 * P.m_a * (va0 * va0 + va1 * va1 + va2 * va2);
+    ic->x[0] = G.sig_r_ion * z[0]; ic->x[1] = G.sig_r_ion * z[1]; ic->x[2] = G.sig_r_ion * z[2];
+    ic->v[0] = G.sig_v_ion * z[3]; ic->v[1] = G.sig_v_ion * z[4]; ic->v[2] = G.sig_v_ion * z[5];
+    ic->x[3] = P.r0 * n0; ic->x[4] = P.r0 * n1; ic->x[5] = P.r0 * n2;
+    ic->v[3] = sign * va0; ic->v[4] = sign * va1; ic->v[5] = sign * va2;
+    ic->phase = (G.phase_mode == 1) ? 6.28318530717958647692 * t[2] : G.phase0;
+}
+
 /* Initial condition of local trajectory j.  Out of line and writing through a pointer on purpose:
  * the struct lives in the stack frame for the duration of a refill only, and the persistent state
  * of the caller stays in registers. */
+template <bool WITH_THERMAL = true> /* false: the caller generates thermal initial conditions itself (bulk kernel) */
 __device__ __forceinline__ void ia_generate_ic(const IaParams &P, const IaGen &G, unsigned long long j, IaIC *ic) {
     if (G.mode == IA_IC_EXPLICIT) {
 #pragma unroll
@@ -76,42 +119,21 @@ __device__ __forceinline__ void ia_generate_ic(const IaParams &P, const IaGen &G
         return;
     }
     const unsigned long long gi = G.first_index + j;
+    if (WITH_THERMAL && G.mode == IA_IC_THERMAL) {
+        /* thermal run (PAPER.md:42,50; reading R18): atom uniform on the r0 sphere, Maxwell-Boltzmann velocity
+         * negated if needed so that v_r < 0; ion Gaussian in position and velocity */
+        double t[14];
+#pragma unroll
+        for (unsigned b = 0; b < 7u; ++b) ia_thermal_task(G, gi, b, t[2 * b], t[2 * b + 1]);
+        ia_thermal_assemble(P, G, t, ic);
+        return;
+    }
     unsigned w0[4], w1[4];
     ia_philox((unsigned)gi, (unsigned)(gi >> 32), G.cell, 0u, (unsigned)G.seed, (unsigned)(G.seed >> 32), w0);
     ia_philox((unsigned)gi, (unsigned)(gi >> 32), G.cell, 1u, (unsigned)G.seed, (unsigned)(G.seed >> 32), w1);
     const double u1 = ia_u53(w0[0], w0[1]), u2 = ia_u53(w0[2], w0[3]);
     const double u3 = ia_u53(w1[0], w1[1]), u4 = ia_u53(w1[2], w1[3]);
     double ct, st, sp, cp;
-    if (G.mode == IA_IC_THERMAL) {
-        /* thermal run (PAPER.md:42,50; reading R18): atom uniform on the r0 sphere, Maxwell-Boltzmann velocity
-         * negated if needed so that v_r < 0; ion Gaussian in position and velocity.  Normal deviates by
-         * Box-Muller on Philox blocks 2..6: (z_2k, z_2k+1) = sqrt(-2 ln u_a) (cos 2 pi u_b, sin 2 pi u_b). */
-        ct = 2.0 * u1 - 1.0;
-        st = sqrt(1.0 - ct * ct);
-        sincospi(2.0 * u2, &sp, &cp);
-        double z[10];
-#pragma unroll
-        for (unsigned b = 2; b <= 6; ++b) {
-            unsigned w[4];
-            ia_philox((unsigned)gi, (unsigned)(gi >> 32), G.cell, b, (unsigned)G.seed, (unsigned)(G.seed >> 32), w);
-            const double R = sqrt(-2.0 * log(ia_u53(w[0], w[1])));
-            double sb, cb;
-            sincospi(2.0 * ia_u53(w[2], w[3]), &sb, &cb);
-            z[2 * (b - 2)] = R * cb;
-            z[2 * (b - 2) + 1] = R * sb;
-        }
-        const double n0 = st * cp, n1 = st * sp, n2 = ct;
-        double va0 = G.sig_v_atom * z[6], va1 = G.sig_v_atom * z[7], va2 = G.sig_v_atom * z[8];
-        const double vr = va0 * n0 + va1 * n1 + va2 * n2;
-        const double sign = (vr > 0.0) ? -1.0 : 1.0;
-        ic->E_au = 0.5 * P.m_a * (va0 * va0 + va1 * va1 + va2 * va2);
-        ic->x[0] = G.sig_r_ion * z[0]; ic->x[1] = G.sig_r_ion * z[1]; ic->x[2] = G.sig_r_ion * z[2];
-        ic->v[0] = G.sig_v_ion * z[3]; ic->v[1] = G.sig_v_ion * z[4]; ic->v[2] = G.sig_v_ion * z[5];
-        ic->x[3] = P.r0 * n0; ic->x[4] = P.r0 * n1; ic->x[5] = P.r0 * n2;
-        ic->v[3] = sign * va0; ic->v[4] = sign * va1; ic->v[5] = sign * va2;
-        ic->phase = (G.phase_mode == 1) ? 6.28318530717958647692 * u3 : G.phase0;
-        return;
-    }
     if (G.mode == IA_IC_GRID) {
         const unsigned long long ii = gi / G.n_phi, jj = gi % G.n_phi;
         /* theta = (i + 1/2) span / n_theta, evaluated as sincospi(theta/pi) */
@@ -213,6 +235,8 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
         double loc_lo[IA_THREADS], loc_hi[IA_THREADS]; /* bracket of the exit localisation (R7) */
         double r2_cur[IA_THREADS];                     /* |d|^2 at the current (last committed) state */
     } sh;
+    /* the fourteen numbers of a thermal initial condition per lane (bulk kernel only) */
+    __shared__ double sh_gen[(LPT == 1 && SRC != IA_SRC_QUEUE) ? IA_THREADS : 1][14];
     double &t_first = sh.t_first[threadIdx.x], &t_last = sh.t_last[threadIdx.x], &phase = sh.phase[threadIdx.x],
            &s_old = sh.s_old[threadIdx.x];
     phase = 0.0; s_old = 0.0;
@@ -276,6 +300,25 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
                     atomicCAS((unsigned long long *)&O.summary->t_first_idle_ns, 0ull, ia_globaltimer());
                 wexh = 1u;
             }
+            /* thermal runs: the seven Philox / Box-Muller tasks of every lane that starts a trajectory, spread over
+             * the warp (ia_thermal_task) */
+            constexpr bool coop_gen = (LPT == 1 && SRC != IA_SRC_QUEUE);
+            if (coop_gen && G.mode == IA_IC_THERMAL) {
+                const bool fresh = got && j >= n_in;
+                const unsigned fm = __ballot_sync(IA_FULL, fresh);
+                const unsigned long long gi_mine = G.first_index + (j - n_in);
+                const unsigned n_tasks = 7u * (unsigned)__popc(fm);
+                for (unsigned t0 = 0; t0 < n_tasks; t0 += 32u) {
+                    const unsigned t = t0 + lane;
+                    const bool act = t < n_tasks;
+                    const unsigned rank = act ? t / 7u : 0u;
+                    const unsigned blk = act ? t - 7u * rank : 0u;
+                    const unsigned owner = __fns(fm, 0u, (int)rank + 1);
+                    const unsigned long long gi_o = __shfl_sync(IA_FULL, gi_mine, (int)(owner & 31u));
+                    if (act) ia_thermal_task(G, gi_o, blk, sh_gen[owner][2u * blk], sh_gen[owner][2u * blk + 1u]);
+                }
+                __syncwarp();
+            }
             if (got) {
                 if (resume || (SRC == IA_SRC_BOTH && j < n_in)) {
                     /* resume a trajectory an earlier kernel handed over */
@@ -301,7 +344,10 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
                 } else if (SRC != IA_SRC_QUEUE) {
                     const unsigned long long jf = j - n_in; /* index within this launch */
                     IaIC ic;
-                    ia_generate_ic(P, G, jf, &ic);
+                    if (coop_gen && G.mode == IA_IC_THERMAL)
+                        ia_thermal_assemble(P, G, sh_gen[coop_gen ? threadIdx.x : 0], &ic);
+                    else
+                        ia_generate_ic<!coop_gen>(P, G, jf, &ic);
                     if (O.ic_dump != nullptr && L.leader) {
                         double *o = O.ic_dump + jf * 14;
 #pragma unroll
@@ -409,9 +455,15 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
                 unsigned long long base = 0;
                 if ((int)lane == first) base = atomicAdd(S.n_out, (unsigned long long)__popc(am));
                 base = __shfl_sync(IA_FULL, base, first);
+                const unsigned long long qidx = base + __popc(am & ((1u << L.gbase) - 1u));
+                if (mode == MODE_RUN && L.valid && qidx >= S.q_cap) {
+                    /* cannot happen (the host sizes the queues for a full grid); never write out of bounds */
+                    if (L.leader) atomicOr(S.fault, 1ull);
+                    mode = MODE_IDLE;
+                }
                 if (mode == MODE_RUN && L.valid) {
                     /* every lane of the group writes the axes it holds, the leader the rest */
-                    IaHand *H = S.q_out + base + __popc(am & ((1u << L.gbase) - 1u));
+                    IaHand *H = S.q_out + qidx;
 #pragma unroll
                     for (int a = 0; a < NA; ++a) {
                         const unsigned ax = L.axis0 + a;
@@ -605,6 +657,8 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
                             if (k < S.late_cap) {
                                 S.late[k].rec = r;
                                 S.late[k].dst = out_rec + slot;
+                            } else {
+                                atomicOr(S.fault, 2ull);
                             }
                         } else {
                             out_rec[slot] = r;

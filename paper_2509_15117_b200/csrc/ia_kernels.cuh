@@ -62,6 +62,8 @@ struct IaSched {
     unsigned long long *n_out;       /* ... counting them here                                           */
     int handoff_lanes;               /* ... once the counter is empty and <= this many trajectories of a warp run */
     unsigned budget;                 /* ... or once it has run this many iterations since the counter ran dry */
+    unsigned long long q_cap;        /* capacity of q_out in entries; an entry beyond it is dropped and ...    */
+    unsigned long long *fault;       /* ... bit 0 of this word set (bit 1: late list full); checked by ia_debug_check */
     unsigned long long *n_fin;       /* non-NULL: counts the trajectories this kernel finishes; a warp hands over  */
     unsigned long long run_floor;    /* ... also once at most this many of the n_in it resumed are still running   */
     unsigned long long warn;

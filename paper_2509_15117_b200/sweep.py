@@ -16,7 +16,6 @@ import json
 import os
 import sys
 
-os.environ.setdefault("CUDA_DEVICE_MAX_CONNECTIONS", "32")
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
@@ -79,8 +78,9 @@ def main():
         if args.t_max_rf > 0.0:
             import dataclasses
             cells = [dataclasses.replace(c, params=dataclasses.replace(c.params, t_max_rf=args.t_max_rf)) for c in cells]
-        # consecutive cells of one (species, trap, D_e, tolerances) cell -- config 4's batches of one Philox stream --
-        # share a ctx and run as one generation: bulk kernels back to back, one straggler chain for all of them
+        # consecutive cells of one (species, trap, D_e, tolerances) cell -- config 4's batches of one Philox stream, the
+        # five temperatures of a thermal species -- share a ctx and run as one pipeline (ia_set_pipeline): the bulk
+        # kernel of a cell first resumes what the cell before left unfinished; one straggler chain at the end
         groups = []
         for cell in cells:
             if groups and groups[-1][0].params == cell.params and len(groups[-1]) < 64:
@@ -115,8 +115,9 @@ def main():
                     "cell": cell.name, "n": n, "seconds": own, "trajectories_per_s": n / own, "rk_steps_per_s": steps / own,
                     "rk_steps": steps, "steps_per_trajectory": steps / n,
                     "bulk_ms": t["bulk_ms"], "chain_ms": t["coop_ms"],
-                    "bulk_frac_of_dfma_peak": FLOP_PER_STEP * (steps - int(s["steps_coop"])) / (t["bulk_ms"] * 1e-3) / 1e12 / peak,
-                    "bulk_lane_efficiency": (steps - int(s["steps_coop"])) / max(int(s["slots_bulk"]), 1),
+                    # steps_kernel: what this cell's bulk kernel executed (its own trajectories and carried ones)
+                    "bulk_frac_of_dfma_peak": FLOP_PER_STEP * int(s["steps_kernel"]) / (t["bulk_ms"] * 1e-3) / 1e12 / peak,
+                    "bulk_lane_efficiency": int(s["steps_kernel"]) / max(int(s["slots_bulk"]), 1),
                     "p_complex": int(s["n_complex"]) / n, "n_status": [int(x) for x in s["n_status"]],
                     "mean_ke_ion_uK": (float(s["sum_ke"]) / max(n_esc, 1)) / KB_EH_PER_K * 1e6,
                     "hist_ncoll": [int(x) for x in s["hist_ncoll"][:12]],
@@ -126,7 +127,7 @@ def main():
                 }
                 print(json.dumps(line), flush=True)
             if len(group) > 1:
-                print(json.dumps({"generation": f"{group[0].name} .. {group[-1].name}", "cells": len(group), "n": n_all,
+                print(json.dumps({"pipeline": f"{group[0].name} .. {group[-1].name}", "cells": len(group), "n": n_all,
                                   "seconds": wall, "trajectories_per_s": n_all / wall, "rk_steps": steps_all,
                                   "rk_steps_per_s": steps_all / wall, "chain_ms": times[0]["coop_ms"],
                                   "bulk_ms_total": sum(t["bulk_ms"] for t in times)}), flush=True)

@@ -767,3 +767,75 @@ def test_maps_from_gpu_records(P):
     assert S.two_proportion_ok(int(g["complex"].sum()), 4096, int(o["complex"].sum()), 4096)[0]
     # the phi = pi/4 saddle line (q_x = -q_y) is complex-dominated: the two columns next to it
     assert g["complex"][:, 31:33].mean() > g["complex"].mean()
+
+
+# ---------------------------------------------------------------------------------------------
+# out-of-bounds writes (SURVEY.md section 5 "sanitizers"; compute-sanitizer is closed on this pool)
+# ---------------------------------------------------------------------------------------------
+def test_no_out_of_bounds_writes_guard_zones(P):
+    """Every path once on small, ragged launches -- bulk only, cooperative only, hand-over at 4/16/32 lanes, a chain
+    with three cooperative levels, a pipelined cycle cut unevenly, pipelined host runs with late records, ia_run_host,
+    the thermal generator -- with guard zones around the caller's output buffers (checked here) and around every
+    buffer the ctx owns (ia_debug_check, which also reads the kernels' fault word and the device-side counts)."""
+    import torch
+    PAD = 4096
+
+    def padded(nbytes):
+        t = torch.full((nbytes + 2 * PAD,), 0x5A, dtype=torch.uint8, device="cuda")
+        return t, t[PAD:PAD + nbytes]
+
+    def intact(t, nbytes):
+        h = t.cpu().numpy()
+        return bool((h[:PAD] == 0x5A).all() and (h[PAD + nbytes:] == 0x5A).all())
+
+    c1 = I.config1(47)                                   # 2,209 trajectories: a ragged last warp
+    c1 = replace(c1, params=replace(c1.params, t_max_rf=40.0))
+    n = c1.launch.n
+    with P.Context(c1.params) as ctx:
+        for path, lanes in ((1, 16), (2, 16), (0, 4), (0, 16), (0, 32)):
+            ctx.set_handoff(lanes)
+            tr, rec = padded(n * P.RECORD_BYTES)
+            ts, summ = padded(P.SUMMARY_BYTES)
+            ti, icb = padded(n * 14 * 8)
+            summ.zero_()
+            P.ia_run(ctx.handle, P.make_launch(replace(c1.launch, path=path)), rec, summ, icb)
+            torch.cuda.synchronize()
+            assert intact(tr, n * 64) and intact(ts, 1024) and intact(ti, n * 112)
+            assert int(P.view_summary(summ)["n_done"]) == n
+            ctx.debug_check()
+        ctx.set_chain(3, 64)
+        _, s3, _ = ctx.run_sync(c1.launch)
+        assert int(s3["n_done"]) == n
+        ctx.debug_check()
+        ctx.set_chain(1, 8192)
+        ctx.set_pipeline(3)
+        cuts = [0, 7, 1500, n]
+        tr, rec = padded(n * P.RECORD_BYTES)
+        sums = [padded(P.SUMMARY_BYTES) for _ in range(3)]
+        for i in range(3):
+            sums[i][1].zero_()
+            ctx.run(replace(c1.launch, n=cuts[i + 1] - cuts[i], first_index=cuts[i]), records=rec[cuts[i] * 64:],
+                    summary=sums[i][1])
+        ctx.join()
+        torch.cuda.synchronize()
+        assert intact(tr, n * 64) and all(intact(t, 1024) for t, _ in sums)
+        assert sum(int(P.view_summary(v)["n_done"]) for _, v in sums) == n
+        ctx.debug_check()
+        host = [(torch.zeros(n * 64, dtype=torch.uint8).pin_memory(), torch.zeros(1024, dtype=torch.uint8).pin_memory())
+                for _ in range(5)]
+        for k, (rh, sh) in enumerate(host):
+            P.ia_submit_host(ctx.handle, P.make_launch(replace(c1.launch, phase0=0.1 * k)), rh, sh)
+        ctx.wait()
+        assert all(int(sh.numpy().view(P.SUMMARY_DTYPE)[0]["n_done"]) == n for _, sh in host)
+        assert all(int((rh.numpy().view(P.RECORD_DTYPE)["steps_acc"] > 0).sum()) == n for rh, _ in host)
+        ctx.debug_check()
+        ctx.set_pipeline(0)
+        _, sh = ctx.run_host(c1.launch)
+        assert int(sh["n_done"]) == n
+        ctx.debug_check()
+    th = I.thermal("Rb87", 1.0, n=1000)
+    th = replace(th, params=replace(th.params, t_max_rf=40.0))
+    with P.Context(th.params) as ctx:
+        _, s, _ = ctx.run_sync(th.launch)
+        assert int(s["n_done"]) == 1000
+        ctx.debug_check()
