@@ -245,6 +245,7 @@ int ia_create(ia_ctx **out, const ia_species *sp, const ia_trap *tr, double De_K
     P.rcsq = T.r_coll_a0 * T.r_coll_a0;
     P.loc_tol = 1e-13 * P.r0sq;
     P.max_steps = T.max_steps;
+    P.n_near = T.t_max_rf > 2.0 ? (unsigned)std::floor(std::fmin(T.t_max_rf - 2.0, 4294967295.0)) : 0u;
     const double d[16] = {P.m_i, P.m_a, P.C4, P.C8, P.De, P.r_e, P.omega, P.T_rf,
                           P.thr, P.h_max, P.h_min, P.t_max, P.r0, P.r_coll, P.rtol, P.atol};
     std::memcpy(c->derived, d, sizeof(d));

@@ -89,6 +89,8 @@ struct IaParams {
     double r0, r0sq, rcsq, loc_tol; /* loc_tol = 1e-13 r0^2 */
     double C4, C8, De, r_e, r_coll, atol;
     unsigned long long max_steps;
+    unsigned n_near; /* the last step is clipped to land on t_max (R5/R8): only looked at from this rf period on */
+    unsigned pad32;
 };
 
 #define IA_DEV __device__ __forceinline__
@@ -426,27 +428,56 @@ IA_DEV void ia_dp5_attempt(const IaParams &P, const IaLane<LPT> &L, const IaVec<
         ia_gather3<LPT>(L, w, W);
         out.s_new = ia_dot3<FUSED>(D, W);
     }
-    /* ode45 norm (R5): per axis the tree (x_i vs v_i), (x_a vs v_a), (ion vs atom); then axis 0 vs 1, then vs 2 */
+    /* ode45 norm (R5): err = max_i |e_i| / max(|y_i|, |ynew_i|, thr) as the pair (num, den) of the component where
+     * the ratio is largest, found by cross-multiplication.  The velocities of this problem (~1e-7 a.u.) lie far below
+     * thr = atol/rtol, so their scale is thr: when that holds for every lane of the warp, the largest velocity ratio is
+     * the largest |e_v| over thr (five compares instead of six three-way scales and six cross-multiplications).  The
+     * general tree is taken otherwise; both give the same pair (the maximum of the same twelve ratios). */
     {
         const double p7 = h * IA_E7;
-        double en[NA], sc[NA];
+        double en[NA], sc[NA], fvi[NA], fva[NA];
+        bool vsmall = true;
 #pragma unroll
         for (int a = 0; a < NA; ++a) {
-            const double fvi = IA_F(p7, N.Ai[a], evi[a]);
-            const double fva = IA_F(p7, N.Aa[a], eva[a]);
-            double n_i = exi[a], d_i = ia_absmax_raw(ia_absmax_raw(Y.xi[a], N.xi[a]), P.thr);
-            ia_ratio_max(n_i, d_i, fvi, ia_absmax_raw(ia_absmax_raw(Y.vi[a], N.vi[a]), P.thr));
-            double n_a = exa[a], d_a = ia_absmax_raw(ia_absmax_raw(Y.xa[a], N.xa[a]), P.thr);
-            ia_ratio_max(n_a, d_a, fva, ia_absmax_raw(ia_absmax_raw(Y.va[a], N.va[a]), P.thr));
-            ia_ratio_max(n_i, d_i, n_a, d_a);
-            en[a] = n_i;
-            sc[a] = d_i;
+            fvi[a] = IA_F(p7, N.Ai[a], evi[a]);
+            fva[a] = IA_F(p7, N.Aa[a], eva[a]);
+            vsmall = vsmall && (fabs(Y.vi[a]) <= P.thr) && (fabs(N.vi[a]) <= P.thr) && (fabs(Y.va[a]) <= P.thr) &&
+                     (fabs(N.va[a]) <= P.thr);
         }
         double EN[3], SC[3];
-        ia_gather3<LPT>(L, en, EN);
-        ia_gather3<LPT>(L, sc, SC);
-        ia_ratio_max(EN[0], SC[0], EN[1], SC[1]);
-        ia_ratio_max(EN[0], SC[0], EN[2], SC[2]);
+        if (__all_sync(IA_FULL, vsmall)) {
+            double ev[NA], EV[3];
+#pragma unroll
+            for (int a = 0; a < NA; ++a) {
+                double n_i = exi[a], d_i = ia_absmax_raw(ia_absmax_raw(Y.xi[a], N.xi[a]), P.thr);
+                ia_ratio_max(n_i, d_i, exa[a], ia_absmax_raw(ia_absmax_raw(Y.xa[a], N.xa[a]), P.thr));
+                en[a] = n_i;
+                sc[a] = d_i;
+                ev[a] = ia_absmax_raw(fvi[a], fva[a]);
+            }
+            ia_gather3<LPT>(L, en, EN);
+            ia_gather3<LPT>(L, sc, SC);
+            ia_gather3<LPT>(L, ev, EV);
+            ia_ratio_max(EN[0], SC[0], EN[1], SC[1]);
+            ia_ratio_max(EN[0], SC[0], EN[2], SC[2]);
+            ia_ratio_max(EN[0], SC[0], ia_absmax_raw(ia_absmax_raw(EV[0], EV[1]), EV[2]), P.thr);
+        } else {
+            /* per axis the tree (x_i vs v_i), (x_a vs v_a), (ion vs atom); then axis 0 vs 1, then vs 2 */
+#pragma unroll
+            for (int a = 0; a < NA; ++a) {
+                double n_i = exi[a], d_i = ia_absmax_raw(ia_absmax_raw(Y.xi[a], N.xi[a]), P.thr);
+                ia_ratio_max(n_i, d_i, fvi[a], ia_absmax_raw(ia_absmax_raw(Y.vi[a], N.vi[a]), P.thr));
+                double n_a = exa[a], d_a = ia_absmax_raw(ia_absmax_raw(Y.xa[a], N.xa[a]), P.thr);
+                ia_ratio_max(n_a, d_a, fva[a], ia_absmax_raw(ia_absmax_raw(Y.va[a], N.va[a]), P.thr));
+                ia_ratio_max(n_i, d_i, n_a, d_a);
+                en[a] = n_i;
+                sc[a] = d_i;
+            }
+            ia_gather3<LPT>(L, en, EN);
+            ia_gather3<LPT>(L, sc, SC);
+            ia_ratio_max(EN[0], SC[0], EN[1], SC[1]);
+            ia_ratio_max(EN[0], SC[0], EN[2], SC[2]);
+        }
         out.err.num = fabs(EN[0]);
         out.err.den = fabs(SC[0]);
     }

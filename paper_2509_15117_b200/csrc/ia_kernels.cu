@@ -228,12 +228,12 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
         unsigned long long slot[IA_THREADS];
         ia_record *rec[IA_THREADS];   /* outputs of the run the group's trajectory belongs to */
         ia_summary *sum[IA_THREADS];
-        unsigned steps_in[IA_THREADS], n_coll[IA_THREADS], n_tp[IA_THREADS], n_loc[IA_THREADS], steps_rej[IA_THREADS],
+        unsigned steps_in[IA_THREADS], n_coll[IA_THREADS], n_tp[IA_THREADS], n_loc[IA_THREADS], att0[IA_THREADS],
             cnt[IA_THREADS], wexh[IA_THREADS], iters[IA_THREADS];
         unsigned flags[IA_THREADS];       /* IA_HAND_LATE | IA_CARRIED */
         unsigned steps_entry[IA_THREADS]; /* attempted steps the trajectory had taken when this kernel got it */
         double loc_lo[IA_THREADS], loc_hi[IA_THREADS]; /* bracket of the exit localisation (R7) */
-        double r2_cur[IA_THREADS];                     /* |d|^2 at the current (last committed) state */
+        double t_fin[IA_THREADS];                      /* time at which the trajectory ended */
     } sh;
     /* the fourteen numbers of a thermal initial condition per lane (bulk kernel only) */
     __shared__ double sh_gen[(LPT == 1 && SRC != IA_SRC_QUEUE) ? IA_THREADS : 1][14];
@@ -245,14 +245,19 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
     ia_summary *&out_sum = sh.sum[threadIdx.x];
     out_rec = O.records; out_sum = O.summary;
     unsigned &steps_in = sh.steps_in[threadIdx.x], &n_coll = sh.n_coll[threadIdx.x], &n_tp = sh.n_tp[threadIdx.x],
-             &n_loc = sh.n_loc[threadIdx.x], &steps_rej = sh.steps_rej[threadIdx.x];
+             &n_loc = sh.n_loc[threadIdx.x];
+    /* attempts are not counted step by step: a running trajectory makes one per iteration of its warp, so the number
+     * it has made is att0 + iters (att0 = attempts before it got here minus the warp's iteration count then) */
+    unsigned &att0 = sh.att0[threadIdx.x];
+    bool s_neg = false;   /* sign of s = d.w at the current state (the value s_old is needed at a bounce only) */
+    bool outside = false; /* |d| >= r0 at the current state: such a trajectory has no exit crossing to localise (R7) */
     unsigned &cnt = sh.cnt[threadIdx.x]; /* warp-uniform: step attempts since the queue ran dry */
     cnt = 0;
     unsigned &iters = sh.iters[threadIdx.x]; /* warp-uniform: step attempts of this warp so far */
     iters = 0;
     unsigned &flags = sh.flags[threadIdx.x], &steps_entry = sh.steps_entry[threadIdx.x];
     flags = 0; steps_entry = 0;
-    t_first = 0.0; t_last = 0.0; slot = 0; steps_in = 0; n_coll = 0; n_tp = 0; n_loc = 0; steps_rej = 0;
+    t_first = 0.0; t_last = 0.0; slot = 0; steps_in = 0; n_coll = 0; n_tp = 0; n_loc = 0; att0 = 0;
     int mode = MODE_IDLE;
     bool failed = false;
     unsigned &wexh = sh.wexh[threadIdx.x]; /* warp-uniform flag: the work counter is empty */
@@ -331,14 +336,16 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
                         Y.Ai[a] = H->A1[ax]; Y.Aa[a] = H->A1[3 + ax];
                     }
                     tf = H->tf; h = H->h; phase = H->phase; s_old = H->s_old;
-                    sh.r2_cur[threadIdx.x] = H->r2_cur;
+                    s_neg = H->s_old < 0.0;
+                    outside = H->r2_cur >= P.r0sq;
                     t_first = H->t_first; t_last = H->t_last; slot = H->slot;
                     out_rec = H->records; out_sum = H->summary;
                     n_per = H->n_per; n_coll = H->n_coll; n_tp = H->n_tp;
-                    steps_acc = H->steps_acc; steps_rej = H->steps_rej; failed = H->failed != 0u;
+                    steps_acc = H->steps_acc; failed = H->failed != 0u;
+                    att0 = H->steps_acc + H->steps_rej - iters;
                     steps_in = H->steps_in;
                     flags = (H->flags & IA_HAND_LATE) | IA_CARRIED;
-                    steps_entry = steps_acc + steps_rej;
+                    steps_entry = H->steps_acc + H->steps_rej;
                     n_loc = 0;
                     mode = MODE_RUN;
                 } else if (SRC != IA_SRC_QUEUE) {
@@ -361,7 +368,8 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
                     slot = jf;
                     out_rec = O.records; out_sum = O.summary;
                     flags = 0; steps_entry = 0;
-                    tf = 0.0; n_per = 0; n_coll = 0; n_tp = 0; steps_acc = 0; steps_rej = 0; n_loc = 0; steps_in = 0;
+                    tf = 0.0; n_per = 0; n_coll = 0; n_tp = 0; steps_acc = 0; n_loc = 0; steps_in = 0;
+                    att0 = 0u - iters;
                     t_first = 0.0; t_last = 0.0; failed = false;
                     phase = ic.phase;
                     bool ok = ia_isfinite(phase);
@@ -409,7 +417,8 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
                         if (h < P.h_min) h = P.h_min;
                         const double W[3] = {ic.v[3] - ic.v[0], ic.v[4] - ic.v[1], ic.v[5] - ic.v[2]};
                         s_old = ia_dot3<true>(D, W);
-                        sh.r2_cur[threadIdx.x] = r2;
+                        s_neg = s_old < 0.0;
+                        outside = r2 >= P.r0sq;
 #pragma unroll
                         for (int a = 0; a < NA; ++a) {
                             const unsigned ax = L.axis0 + a;
@@ -473,8 +482,9 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
                     }
                     if (L.leader) {
                         const bool carried = (flags & IA_CARRIED) != 0u;
+                        const unsigned attempts = att0 + iters;
                         H->tf = tf; H->h = h; H->phase = phase; H->s_old = s_old;
-                        H->r2_cur = sh.r2_cur[threadIdx.x];
+                        H->r2_cur = outside ? P.r0sq : 0.0; /* only whether it is beyond r0 matters (R7) */
                         H->t_first = t_first; H->t_last = t_last; H->slot = slot;
                         /* a trajectory of a pipelined host run leaves with the HOST address of its record array */
                         const bool to_host = !carried && S.late_dst != nullptr;
@@ -482,12 +492,12 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
                         H->flags = to_host ? IA_HAND_LATE : (flags & IA_HAND_LATE);
                         H->summary = out_sum;
                         H->n_per = n_per; H->n_coll = n_coll; H->n_tp = n_tp;
-                        H->steps_acc = steps_acc; H->steps_rej = steps_rej; H->failed = failed ? 1u : 0u;
+                        H->steps_acc = steps_acc; H->steps_rej = attempts - steps_acc; H->failed = failed ? 1u : 0u;
                         /* steps taken before the first hand-over */
-                        H->steps_in = carried ? steps_in : steps_acc + steps_rej;
+                        H->steps_in = carried ? steps_in : attempts;
                         if (SRC != IA_SRC_QUEUE && O.summary != nullptr)
                             atomicAdd((unsigned long long *)&O.summary->steps_kernel,
-                                      (unsigned long long)(steps_acc + steps_rej - steps_entry));
+                                      (unsigned long long)(attempts - steps_entry));
                     }
                     mode = MODE_IDLE;
                 }
@@ -501,70 +511,117 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
         /* ---- the step loop proper: up to IA_INNER attempts without looking at the counter, the queues or the
          * budget; it is left as soon as a trajectory of the warp terminates.  Everything that is only needed
          * between two visits here stays out of its registers. ---- */
-        int fin;          /* >= 0: terminate with this status */
-        double t_fin;
-        bool fin_exit;
+        int fin;          /* >= 0: terminate with this status (0: at the localised exit, i.e. at state N) */
+        double &t_fin = sh.t_fin[threadIdx.x]; /* written when a trajectory ends: kept out of the loop's registers */
         IaVec<LPT> N;
         unsigned it = 0;
+        /* R5, status 4: the loop never takes a trajectory past max_steps attempts.  Attempts are not counted per
+         * step: a running trajectory makes one per iteration of its warp, so their number is att0 + iters. */
+        unsigned inner = IA_INNER;
+        {
+            unsigned long long left = ~0ull;
+            if (mode == MODE_RUN) {
+                const unsigned long long done = (unsigned long long)(att0 + iters);
+                left = P.max_steps > done ? P.max_steps - done : 1ull;
+            }
+            inner = __reduce_min_sync(IA_FULL, (unsigned)(left < (unsigned long long)IA_INNER ? left : IA_INNER));
+        }
         do {
         /* one DP5(4) attempt for every lane (idle lanes step a harmless dummy state) */
         const bool run = (mode == MODE_RUN), loc = (mode == MODE_LOC);
-        /* clip the last step to land on t_max (R5/R8) */
-        const double rem = (P.t_max_rf - (double)n_per) * P.T_rf - tf;
-        const bool last = run && (h >= rem);
-        h = last ? rem : h;
+        /* clip the last step to land on t_max (R5/R8): only within the last two rf periods */
+        bool last = false;
+        if (run && n_per >= P.n_near) {
+            const double rem = (P.t_max_rf - (double)n_per) * P.T_rf - tf;
+            last = h >= rem;
+            h = last ? rem : h;
+        }
         IaStepOut so;
         ia_dp5_attempt<LPT, true>(P, L, Y, tf, phase, h, N, so);
 
-        /* ---- controller, events, termination: straight-line selects; rare cases branch ---- */
+        /* ---- controller (R5): straight-line selects; everything that happens once per bounce or per trajectory
+         * (turning points, exit, localisation, termination) sits in one branch ---- */
         const double hs = h; /* the step just attempted */
         const double denr = P.rtol * so.err.den;
         const bool accept = so.finite && (so.err.num <= denr);
-        double xr = so.err.num * ia_rcp(denr); /* err / rtol */
-        xr = so.finite ? xr : 1e30;
-        xr = ia_max(ia_min(xr, 1e30), 1e-30); /* NaN -> 1e30 (ia_min returns its second operand then) */
-        const double fac = 0.8 * ia_inv_fifth_root(xr); /* 0.8 (rtol/err)^(1/5) */
-        const double now = (double)n_per * P.T_rf + tf;
-        const double g = so.r2n - P.r0sq;
-        const bool g_small = fabs(g) <= P.loc_tol;
+        /* 0.8 (rtol/err)^(1/5).  err = 0 gives NaN and err = NaN or inf gives NaN or 0: ia_min / ia_max below return
+         * their second operand then, i.e. growth by 5 and shrinkage by 10 as the step law says */
+        const double fac = 0.8 * ia_inv_fifth_root(so.err.num * ia_rcp(denr));
         const bool acc = run && accept, rej = run && !accept;
         steps_acc += acc ? 1u : 0u;
-        if (rej) ++steps_rej;
-        /* events (R6): sign changes of s = d.w at accepted-step ends */
-        const double s_prev = s_old;
-        const bool neg_old = s_prev < 0.0, neg_new = so.s_new < 0.0;
-        const bool flip = acc && (neg_old != neg_new);
-        if (flip) {
-            ++n_tp;
-            if (neg_old && so.r2n < P.rcsq) { /* a minimum of r(t) at short range: a bounce */
-                const double tc = now + (hs * s_prev) * ia_rcp(s_prev - so.s_new);
-                if (n_coll == 0u) t_first = tc;
-                t_last = tc;
-                ++n_coll;
+        const bool neg_new = so.s_new < 0.0;
+        const bool flip = acc && (neg_new != s_neg); /* events (R6): sign changes of s = d.w at accepted-step ends */
+        /* exit (R7): first upward crossing of |d| = r0 */
+        const bool exitc = acc && (so.r2n > P.r0sq) && (so.s_new > 0.0);
+        const bool commit = acc && !exitc;
+        fin = -1;
+        if (flip || exitc || loc || (commit && last) || (rej && hs <= P.h_min)) {
+            const double now = (double)n_per * P.T_rf + tf; /* t_n: nothing is committed yet */
+            if (flip) {
+                ++n_tp;
+                if (s_neg && so.r2n < P.rcsq) { /* a minimum of r(t) at short range: a bounce */
+                    const double s_prev = s_old;
+                    const double tc = now + (hs * s_prev) * ia_rcp(s_prev - so.s_new);
+                    if (n_coll == 0u) t_first = tc;
+                    t_last = tc;
+                    ++n_coll;
+                }
+            }
+            if (exitc || loc) {
+                /* localisation by bracketed Newton on g(hk) = |d(t_n + hk)|^2 - r0^2 over uncontrolled steps from
+                 * (t_n, y_n).  A trajectory that was already outside at t_n (a thermal start beyond r0 that never
+                 * came in) has no crossing to localise: it ends with the detecting step */
+                const double g = so.r2n - P.r0sq;
+                const bool g_small = fabs(g) <= P.loc_tol;
+                bool fin_exit;
+                if (loc) {
+                    ++n_loc;
+                    fin_exit = g_small || n_loc >= 60u;
+                } else {
+                    fin_exit = g_small || outside;
+                }
+                if (!fin_exit) {
+                    /* Newton kept inside the bracket [lo, hi] of step sizes: g(hi) > 0 is known, lo = 0 where the
+                     * trajectory was still inside.  A proposal that leaves the bracket (near-tangential exit,
+                     * d.w ~ 0) is replaced by the midpoint -- one uncontrolled step of many rf periods would blow
+                     * the ion's state up.  NaN compares false and ends in the midpoint too. */
+                    double lo = 0.0, hi = hs;
+                    if (exitc) {
+                        n_loc = 0u;
+                    } else {
+                        lo = sh.loc_lo[threadIdx.x];
+                        hi = sh.loc_hi[threadIdx.x];
+                        if (g > 0.0) hi = hs; else lo = hs;
+                    }
+                    double hn = hs - g * ia_rcp(2.0 * so.s_new);
+                    if (!(so.s_new > 0.0 && hn > lo && hn < hi)) hn = 0.5 * (lo + hi);
+                    h = hn; /* neither accepted-and-committed nor rejected: the step law below leaves it alone */
+                    sh.loc_lo[threadIdx.x] = lo;
+                    sh.loc_hi[threadIdx.x] = hi;
+                    mode = MODE_LOC;
+                } else {
+                    fin = 0;
+                    t_fin = now + hs;
+                }
+            }
+            if (fin == 0) {
+                /* ended at the localised exit */
+            } else if (commit && last) {
+                fin = 1;
+                t_fin = P.t_max;
+            } else if (rej && hs <= P.h_min) {
+                fin = 2;
+                t_fin = now;
             }
         }
-        /* exit (R7): first upward crossing of |d| = r0, localised by bracketed Newton on
-         * g(hk) = |d(t_n + hk)|^2 - r0^2 over uncontrolled steps from (t_n, y_n) */
-        const bool exitc = acc && (so.r2n > P.r0sq) && (so.s_new > 0.0);
-        /* a trajectory that was already outside at t_n (a thermal start beyond r0 that never came in) has no
-         * crossing to localise: it ends with the detecting step */
-        bool no_root = false;
-        if (exitc) no_root = sh.r2_cur[threadIdx.x] >= P.r0sq;
-        bool loc_done = false;
-        if (loc) {
-            ++n_loc;
-            loc_done = g_small || n_loc >= 60u;
-        }
-        fin_exit = (exitc && (g_small || no_root)) || loc_done;
-        const bool newton = (exitc && !g_small && !no_root) || (loc && !loc_done);
-        const bool commit = acc && !exitc;
-        const bool underflow = rej && (hs <= P.h_min);
         /* commit the accepted step: y <- ynew, k1 <- k7 (FSAL), t <- t + h with the time kept folded (R9) */
         {
             const double tfn = tf + hs;
-            const bool wrap = tfn >= P.T_rf;
-            tf = commit ? (wrap ? tfn - P.T_rf : tfn) : tf;
-            n_per += (commit && wrap) ? 1u : 0u;
+            tf = commit ? tfn : tf;
+            if (commit && tfn >= P.T_rf) {
+                tf = tfn - P.T_rf;
+                ++n_per;
+            }
 #pragma unroll
             for (int a = 0; a < NA; ++a) {
                 Y.xi[a] = commit ? N.xi[a] : Y.xi[a];
@@ -574,56 +631,25 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
                 Y.Ai[a] = commit ? N.Ai[a] : Y.Ai[a];
                 Y.Aa[a] = commit ? N.Aa[a] : Y.Aa[a];
             }
-            if (commit) {
-                s_old = so.s_new;
-                sh.r2_cur[threadIdx.x] = so.r2n;
-            }
+            if (commit) s_old = so.s_new; /* its value is read at the next bounce only; its sign is s_neg */
+            s_neg = commit ? neg_new : s_neg;
+            outside = commit ? (so.r2n >= P.r0sq) : outside;
         }
         /* step size of the next attempt (R5) */
         {
             const double h_acc = ia_min(failed ? hs : hs * ia_min(fac, 5.0), P.h_max);
             const double h_rej = ia_max(failed ? 0.5 * hs : hs * ia_max(fac, 0.1), P.h_min);
-            h = commit ? h_acc : (rej ? h_rej : hs);
+            h = commit ? h_acc : (rej ? h_rej : h);
             failed = commit ? false : (rej ? true : failed);
         }
-        if (newton) {
-            /* Newton on g kept inside the bracket [lo, hi] of step sizes from (t_n, y_n): g(hi) > 0 is known,
-             * lo = 0 where the trajectory was still inside.  A proposal that leaves the bracket (near-tangential
-             * exit, d.w ~ 0) is replaced by the midpoint -- one uncontrolled step of many rf periods would blow
-             * the ion's state up.  NaN compares false and ends in the midpoint too. */
-            double lo = 0.0, hi = hs;
-            if (exitc) {
-                n_loc = 0u;
-            } else {
-                lo = sh.loc_lo[threadIdx.x];
-                hi = sh.loc_hi[threadIdx.x];
-                if (g > 0.0) hi = hs; else lo = hs;
-            }
-            double hn = hs - g * ia_rcp(2.0 * so.s_new);
-            if (!(so.s_new > 0.0 && hn > lo && hn < hi)) hn = 0.5 * (lo + hi);
-            h = hn;
-            sh.loc_lo[threadIdx.x] = lo;
-            sh.loc_hi[threadIdx.x] = hi;
-            mode = MODE_LOC;
-        }
-        fin = -1;
-        t_fin = now + hs;
-        if (fin_exit) {
-            fin = 0;
-        } else if (commit && last) {
-            fin = 1;
-            t_fin = P.t_max;
-        } else if (underflow) {
-            fin = 2;
-            t_fin = now;
-        } else if (run && !newton && (unsigned long long)steps_acc + (unsigned long long)steps_rej >= P.max_steps) {
+        ++it;
+        } while (!__any_sync(IA_FULL, fin >= 0) && it < inner);
+        cnt += it;
+        iters += it;
+        if (fin < 0 && mode == MODE_RUN && (unsigned long long)(att0 + iters) >= P.max_steps) {
             fin = 4;
             t_fin = (double)n_per * P.T_rf + tf;
         }
-        ++it;
-        } while (!__any_sync(IA_FULL, fin >= 0) && it < IA_INNER);
-        cnt += it;
-        iters += it;
 
         if (__any_sync(IA_FULL, fin >= 0)) {
             /* observables (R10) + record (a10) + ensemble reduction (a11); the velocity vectors of the
@@ -631,8 +657,8 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
             double wi[NA], wa[NA], VI[3], VA[3];
 #pragma unroll
             for (int a = 0; a < NA; ++a) {
-                wi[a] = fin_exit ? N.vi[a] : Y.vi[a];
-                wa[a] = fin_exit ? N.va[a] : Y.va[a];
+                wi[a] = (fin == 0) ? N.vi[a] : Y.vi[a];
+                wa[a] = (fin == 0) ? N.va[a] : Y.va[a];
             }
             ia_gather3<LPT>(L, wi, VI);
             ia_gather3<LPT>(L, wa, VA);
@@ -640,6 +666,7 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
                 if (L.leader) {
                     const double ke = (0.5 * P.m_i) * ia_dot3<true>(VI, VI);
                     const bool carried = (flags & IA_CARRIED) != 0u;
+                    const unsigned steps_rej = att0 + iters - n_loc - steps_acc; /* attempts that were not accepted */
                     if (out_rec != nullptr) {
                         ia_record r;
                         r.ke_ion = ke;
