@@ -51,7 +51,8 @@ __device__ __forceinline__ void ia_philox(unsigned c0, unsigned c1, unsigned c2,
     out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
-/* 53-bit uniform in (0,1) from two words (reading R2) */
+/* 53-bit uniform from two words (reading R2): (k + 1/2) 2^-53 for k < 2^52; from 2^52 on the sum k + 1/2 ties to even, so
+ * the map is onto (0, 1] -- u = 1 for the one word pair with all 53 bits set (pinned on the oracle side) */
 __device__ __forceinline__ double ia_u53(unsigned we, unsigned wo) {
     return ((double)(we >> 5) * 67108864.0 + (double)(wo >> 6) + 0.5) * (1.0 / 9007199254740992.0);
 }

@@ -4,9 +4,9 @@
 
 The step loop is the innermost loop that contains the Runge-Kutta attempt: the backward branch with the smallest
 span among those that enclose at least six MUFU.RCP64H (one reciprocal per stage).  Prints the FP64-pipe count
-(DFMA + DMUL + DADD + DSETP), the other opcodes, local-memory instructions (LDL / STL: spills, must be 0) and the
-issue-slot model of DESIGN.md "Roofline" (an FP64 instruction holds the issue port of its SM sub-partition for two
-cycles, any other instruction for one).  Reporting only: nothing here is used by the library.
+(DFMA + DMUL + DADD + DSETP), the other opcodes and the local-memory instructions (LDL / STL: spills, must be 0).
+The count is static: rarely taken branches inside the loop are included.  Reporting only: nothing here is used by the
+library.
 """
 from __future__ import annotations
 
@@ -63,8 +63,11 @@ def main():
                                                          if k not in ("DFMA", "DMUL", "DADD", "DSETP")))
     print(f"  local memory in the whole kernel: {whole['LDL']} LDL, {whole['STL']} STL")
     print(f"  flops per attempted step counted from SASS: {2 * hist['DFMA'] + hist['DMUL'] + hist['DADD']}")
-    print(f"  issue slots per warp and step: 2 x {fp64} + {len(body) - fp64} = {2 * fp64 + len(body) - fp64}"
-          f" -> FP64 pipe busy at most {2 * fp64 / (2 * fp64 + len(body) - fp64):.3f} of the time")
+    print(f"  STATIC count: the loop body holds both branches of the error norm (the general tree is not taken in these "
+          f"units) and the rarely taken event / termination branch; the instructions a step executes are counted by "
+          f"ncu (profiles/r02b_k1_ncu.md)")
+    print(f"  issue slots if every instruction of the body ran: 2 x {fp64} + {len(body) - fp64} = "
+          f"{2 * fp64 + len(body) - fp64}")
 
 
 if __name__ == "__main__":

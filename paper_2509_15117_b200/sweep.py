@@ -2,7 +2,7 @@
 cell: ensemble results (complex-formation probability, mean ion energy gain, collision-count histogram, survival) and
 device times of the two kernels from the library's own CUDA events.
 
-    python -m paper_2509_15117_b200.sweep --configs 0,2,3:0:10,4,thermal [--scale 1.0]
+    python -m paper_2509_15117_b200.sweep --configs 0,2,3:0:10,4,thermal,fig4 [--scale 1.0] [--concurrent] [--lengths]
 
 A config may carry a slice of its cells (3:0:10 = cells 0..9 of config 3: the D_e = 0.1 K and 1 K rows).
 
@@ -47,6 +47,12 @@ def cells_of(which: str, scale: float):
         return [shrink(c) for c in I.config3()]
     if which == "4":
         return [shrink(c) for c in I.config4()]
+    if which == "fig4":
+        # Fig. 4's radius r0 = 20 000 a0 at 10 uK for the four species of the figure with a
+        # random rf phase, and Rb with the phase fixed at 0 and at pi
+        cells = [I.fig4(sp, 10.0, n=2 ** 20) for sp in ("Li7", "Na23", "K39", "Rb87")]
+        cells += [I.fig4("Rb87", 10.0, n=2 ** 20, phase_mode=0, phase0=ph) for ph in (0.0, float(np.pi))]
+        return [shrink(c) for c in cells]
     if which == "thermal":
         return [shrink(I.thermal(sp, T, De)) for De in (1.0, 100.0) for sp in I.SPECIES_ORDER for T in I.THERMAL_T_UK]
     raise SystemExit(f"unknown config {which}")
@@ -59,6 +65,12 @@ def main():
     ap.add_argument("--t-max-rf", type=float, default=0.0,
                     help="override every cell's time limit (rf periods): bounds the straggler chain; complexes still "
                          "bound then are counted as such (status 1)")
+    ap.add_argument("--lengths", action="store_true",
+                    help="also print, per cell, the distribution of trajectory lengths (attempted steps) read from the "
+                         "records: share of trajectories and of the work beyond 2^k steps")
+    ap.add_argument("--concurrent", action="store_true",
+                    help="enqueue every group of cells (one ctx each) on a stream of its own before waiting for any: "
+                         "the straggler chains of cells with different parameters then overlap")
     ap.add_argument("--device", type=int, default=0)
     args = ap.parse_args()
     import torch
@@ -87,19 +99,25 @@ def main():
                 groups[-1].append(cell)
             else:
                 groups.append([cell])
-        for group in groups:
-            with P.Context(group[0].params, device=args.device) as ctx:
-                ctx.set_pipeline(len(group) if len(group) > 1 else 0)
-                bufs = [ctx.alloc(c.launch.n) for c in group]
-                ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        def enqueue(group, stream):
+            """one ctx per group; every run and the join enqueued on `stream`, nothing waited for"""
+            ctx = P.Context(group[0].params, device=args.device)
+            ctx.set_pipeline(len(group) if len(group) > 1 else 0)
+            ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            with torch.cuda.stream(stream):
+                bufs = [ctx.alloc(c.launch.n) for c in group]   # zero-filled on the stream the kernels run on
                 ev0.record()
                 for c, (rec, summ, _) in zip(group, bufs):
                     ctx.run(c.launch, records=rec, summary=summ)
                 ctx.join()
                 ev1.record()
-                torch.cuda.synchronize()
-                times = [ctx.timing(len(group) - 1 - k) for k in range(len(group))]
-                T_rf = ctx.derived["T_rf"]
+            return ctx, bufs, ev0, ev1
+
+        def report(group, ctx, bufs, ev0, ev1):
+            ev1.synchronize()
+            times = [ctx.timing(len(group) - 1 - k) for k in range(len(group))]
+            T_rf = ctx.derived["T_rf"]
+            ctx.close()
             wall = ev0.elapsed_time(ev1) * 1e-3
             n_all = steps_all = 0
             for cell, (rec, summ, _), t in zip(group, bufs, times):
@@ -110,7 +128,7 @@ def main():
                 steps_all += steps
                 n_esc = int(s["n_status"][0])
                 tt, S = Ob.survival_curve(s, T_rf)
-                own = wall if len(group) == 1 else float("nan")   # a generation shares its wall time
+                own = wall if len(group) == 1 else float("nan")   # the cells of a pipeline share its wall time
                 line = {
                     "cell": cell.name, "n": n, "seconds": own, "trajectories_per_s": n / own, "rk_steps_per_s": steps / own,
                     "rk_steps": steps, "steps_per_trajectory": steps / n,
@@ -126,12 +144,43 @@ def main():
                     "n_handoff": int(s["n_handoff"]), "warn": int(s["warn"]),
                 }
                 print(json.dumps(line), flush=True)
+                if args.lengths:
+                    r = P.view_records(rec, n)
+                    st = r["steps_acc"].astype(np.int64) + r["steps_rej"] + r["n_loc"]
+                    tot = float(st.sum())
+                    rows = {}
+                    for k in range(9, 25):
+                        m = st >= (1 << k)
+                        rows[f"2^{k}"] = {"trajectories": float(m.mean()), "work": float(st[m].sum() / tot),
+                                          "work_beyond": float((st[m] - (1 << k)).sum() / tot)}
+                    tm = r["status"] == 1
+                    print(json.dumps({"cell": cell.name, "lengths": {
+                        "mean": tot / n, "median": float(np.median(st)), "max": int(st.max()), "beyond": rows,
+                        "at_t_max": int(tm.sum()), "at_t_max_steps_min_mean_max":
+                            [int(st[tm].min()), float(st[tm].mean()), int(st[tm].max())] if tm.any() else None}}), flush=True)
             if len(group) > 1:
                 print(json.dumps({"pipeline": f"{group[0].name} .. {group[-1].name}", "cells": len(group), "n": n_all,
                                   "seconds": wall, "trajectories_per_s": n_all / wall, "rk_steps": steps_all,
                                   "rk_steps_per_s": steps_all / wall, "chain_ms": times[0]["coop_ms"],
                                   "bulk_ms_total": sum(t["bulk_ms"] for t in times)}), flush=True)
-            del bufs
+
+        if args.concurrent:
+            # Cells with different parameters cannot share a pipeline, but their straggler chains can share the GPU: a
+            # chain ends as a few hundred warps that wait on their own dependent chains, so the chains of all groups --
+            # each on a stream of its own -- overlap one another and the bulk kernels of the groups enqueued later
+            t0 = torch.cuda.Event(enable_timing=True)
+            t1 = torch.cuda.Event(enable_timing=True)
+            t0.record()
+            inflight = [(g, *enqueue(g, torch.cuda.Stream())) for g in groups]
+            for g, ctx, bufs, ev0, ev1 in inflight:
+                report(g, ctx, bufs, ev0, ev1)
+            t1.record()
+            torch.cuda.synchronize()
+            print(json.dumps({"concurrent_groups": len(groups), "config": which, "seconds": t0.elapsed_time(t1) * 1e-3,
+                              "n": sum(c.launch.n for g in groups for c in g)}), flush=True)
+        else:
+            for group in groups:
+                report(group, *enqueue(group, torch.cuda.current_stream()))
 
 
 if __name__ == "__main__":
