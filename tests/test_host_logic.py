@@ -234,3 +234,51 @@ def test_summary_reduction_over_two_gloo_ranks():
         assert tot["steps_acc"] == int(a["steps_acc"]) + int(b["steps_acc"])
         assert abs(tot["sum_ke"] - (a["sum_ke"] + b["sum_ke"])) < 1e-15
     assert (res[0][3], res[0][4], res[1][3], res[1][4]) == (0, 501, 501, 500)
+
+
+def test_fig4_cells_and_summary_sums():
+    """ia_inputs.fig4: r0 = 20 000 a0, D_e = 1 K, octant directions, random or fixed phase, a Philox cell of
+    its own; sweep lists the six cells of profiles/r02_summary.md section 8; dist.sum_summaries adds field by field."""
+    import paper_2509_15117_b200 as P
+    from paper_2509_15117_b200 import sweep
+    c = I.fig4("Rb87", 10.0, n=100)
+    assert c.params.r0_a0 == 20000.0 and c.params.De_K == 1.0 and c.params.m_atom_u == I.ATOMS["Rb87"]["m_u"]
+    assert c.launch.mode == I.MODE_PHILOX and c.launch.domain == 0 and c.launch.phase_mode == 1
+    assert c.launch.E_min_uK == c.launch.E_max_uK == 10.0
+    f = I.fig4("Rb87", 10.0, n=100, phase_mode=0, phase0=1.25)
+    assert f.launch.phase_mode == 0 and f.launch.phase0 == 1.25 and f.launch.cell == c.launch.cell and f.name != c.name
+    used = {x.launch.cell for x in I.config2(8) + I.config3(8) + I.config4(64, 64)} | \
+           {I.thermal(sp, T, De).launch.cell for De in (1.0, 100.0) for sp in I.SPECIES_ORDER for T in I.THERMAL_T_UK}
+    assert not used & {I.fig4(sp).launch.cell for sp in I.SPECIES_ORDER}
+    cells = sweep.cells_of("fig4", 1.0)
+    assert len(cells) == 6 and sum(x.launch.phase_mode == 0 for x in cells) == 2
+    arr = np.zeros(3, dtype=P.SUMMARY_DTYPE)
+    arr["n_done"] = [1, 2, 3]
+    arr["hist_ncoll"][:, 1] = [5, 6, 7]
+    arr["steps_kernel"] = [10, 20, 30]
+    arr["sum_ke"] = [0.5, 0.25, 0.125]
+    tot = D.sum_summaries(arr)
+    assert int(tot["n_done"]) == 6 and int(tot["hist_ncoll"][1]) == 18 and int(tot["steps_kernel"]) == 60
+    assert float(tot["sum_ke"]) == 0.875
+    assert "steps_kernel" in D._SUM_FIELDS
+
+
+def test_persistent_kernels_use_no_local_memory():
+    """BASELINE.json north_star: register spills must be zero.  Checked on the built library itself: the SASS of the
+    two persistent kernels holds no LDL / STL at all (no stack frame, no spill), and the step loop is where the
+    histogram tool says it is (an FP64-dominated loop with seven reciprocals)."""
+    import shutil
+    if shutil.which("cuobjdump") is None:
+        pytest.skip("cuobjdump not on PATH")
+    import paper_2509_15117_b200 as P
+    from paper_2509_15117_b200 import sass_histogram as H
+    P.load()
+    for kernel, fp64_min in (("bulk", 550), ("coop", 280)):
+        ins = H.instructions(kernel)
+        assert len(ins) > 1000
+        ops = [t.split()[0].split(".")[0] for _, t in ins]
+        assert "LDL" not in ops and "STL" not in ops
+        lo, hi, body = H.step_loop(ins)
+        n64 = sum(t.split()[0].split(".")[0] in ("DFMA", "DMUL", "DADD", "DSETP") for t in body)
+        assert n64 >= fp64_min and n64 > 0.4 * len(body)
+        assert sum(t.startswith("MUFU.RCP64H") for t in body) >= 7
