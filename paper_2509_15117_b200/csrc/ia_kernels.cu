@@ -231,6 +231,8 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
         ia_summary *sum[IA_THREADS];
         unsigned steps_in[IA_THREADS], n_coll[IA_THREADS], n_tp[IA_THREADS], n_loc[IA_THREADS], att0[IA_THREADS],
             cnt[IA_THREADS], wexh[IA_THREADS], iters[IA_THREADS];
+        unsigned per_fin[IA_THREADS];     /* warp-uniform: 16 x running mean of the iterations per finished trajectory */
+        unsigned last_fin[IA_THREADS];    /* warp-uniform: iteration count at the last finish */
         unsigned flags[IA_THREADS];       /* IA_HAND_LATE | IA_CARRIED */
         unsigned steps_entry[IA_THREADS]; /* attempted steps the trajectory had taken when this kernel got it */
         double loc_lo[IA_THREADS], loc_hi[IA_THREADS]; /* bracket of the exit localisation (R7) */
@@ -258,6 +260,8 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
     iters = 0;
     unsigned &flags = sh.flags[threadIdx.x], &steps_entry = sh.steps_entry[threadIdx.x];
     flags = 0; steps_entry = 0;
+    sh.per_fin[threadIdx.x] = 16u * 1024u; /* start from "long trajectories": no waiting until finishes say otherwise */
+    sh.last_fin[threadIdx.x] = 0u;
     t_first = 0.0; t_last = 0.0; slot = 0; steps_in = 0; n_coll = 0; n_tp = 0; n_loc = 0; att0 = 0;
     int mode = MODE_IDLE;
     bool failed = false;
@@ -285,9 +289,22 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
 
     for (;;) {
         const bool was_exh = wexh != 0u;
-        /* ---- refill idle groups from the global work counter (a12) ---- */
+        /* ---- refill idle groups from the global work counter (a12) ----
+         * Starting a trajectory costs the whole warp ~1e3 instructions (generator, first acceleration, first step
+         * size), an idle lane ~27 per step it sits out.  When trajectories are short (thermal bars: 100-400 steps, one
+         * of the warp's 32 ends every few steps) it pays to let a few lanes idle and start several together: with I
+         * the warp's iterations per finished trajectory (running mean), B = floor(sqrt(K / I)) lanes are collected,
+         * K = 111 for the thermal generator, 59 otherwise -- B = 1 (no waiting) from ~900 resp. ~1900 steps per
+         * trajectory on.  Which lane runs which index changes, no trajectory does. */
         const bool want = L.valid && (mode == MODE_IDLE) && !wexh;
-        const unsigned wm = __ballot_sync(IA_FULL, want && L.leader);
+        unsigned wm = __ballot_sync(IA_FULL, want && L.leader);
+        if (!resume && wm != 0u) {
+            const unsigned I = max(sh.per_fin[threadIdx.x] >> 4, 1u); /* 1/16 iterations, warp-uniform */
+            const unsigned K = (G.mode == IA_IC_THERMAL) ? 111u : 59u;
+            unsigned B = 1u;
+            while (B < 8u && (B + 1u) * (B + 1u) * I <= K) ++B;
+            if ((unsigned)__popc(wm) < B && __any_sync(IA_FULL, mode != MODE_IDLE)) wm = 0u;
+        }
         if (wm) {
             const int first = __ffs(wm) - 1;
             unsigned long long base = 0;
@@ -653,6 +670,12 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
         }
 
         if (__any_sync(IA_FULL, fin >= 0)) {
+            {   /* iterations per finished trajectory, running mean with weight 1/4 (for the refill rule above) */
+                const unsigned nf = (unsigned)__popc(__ballot_sync(IA_FULL, fin >= 0 && L.leader));
+                const unsigned per = 16u * min(iters - sh.last_fin[threadIdx.x], 4096u) / max(nf, 1u);
+                sh.per_fin[threadIdx.x] = (3u * sh.per_fin[threadIdx.x] + per) >> 2;
+                sh.last_fin[threadIdx.x] = iters;
+            }
             /* observables (R10) + record (a10) + ensemble reduction (a11); the velocity vectors of the
              * terminating state are gathered by the whole warp, the group leader writes */
             double wi[NA], wa[NA], VI[3], VA[3];

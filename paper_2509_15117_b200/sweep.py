@@ -32,10 +32,14 @@ def cells_of(which: str, scale: float):
     import ia_inputs as I
 
     def shrink(c):
+        """--scale: trajectories per cell = scale x the cell's own size (at least 1024); a scale above 1 only for the
+        cells that are not pieces of one index stream (thermal bars at Fig. 3's 10^7: --scale 9.5367)"""
         n = max(1024, int(round(scale * c.launch.n)))
         if c.launch.mode == I.MODE_GRID:
             return c
-        return dataclasses.replace(c, launch=dataclasses.replace(c.launch, n=min(n, c.launch.n)))
+        if scale > 1.0 and which == "4":
+            raise SystemExit("--scale > 1 would make config 4's batches overlap")
+        return dataclasses.replace(c, launch=dataclasses.replace(c.launch, n=n))
     if which == "0":
         return [I.config0()]
     if which == "1":
@@ -171,7 +175,10 @@ def main():
             t0 = torch.cuda.Event(enable_timing=True)
             t1 = torch.cuda.Event(enable_timing=True)
             t0.record()
-            inflight = [(g, *enqueue(g, torch.cuda.Stream())) for g in groups]
+            inflight = []
+            for g in groups:
+                inflight.append((g, *enqueue(g, torch.cuda.Stream())))
+                print(f"enqueued {g[0].name} ({len(inflight)} of {len(groups)})", file=sys.stderr, flush=True)
             for g, ctx, bufs, ev0, ev1 in inflight:
                 report(g, ctx, bufs, ev0, ev1)
             t1.record()
