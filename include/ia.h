@@ -140,7 +140,8 @@ typedef struct {
 #define IA_HIST_BINS 32
 #define IA_LIFE_BINS 64
 /* Ensemble reduction of one launch (R16, R17), 1024 bytes.  The library
- * ACCUMULATES into it: the caller zeroes it before the first launch it should cover. */
+ * ACCUMULATES into it: the caller zeroes it before the first launch it should cover -- on the stream the
+ * launch is enqueued on, or ordered before it (a zero-fill on another stream races with the kernels). */
 typedef struct {
     uint64_t n_done;            /* trajectories finished                                            */
     uint64_t n_status[5];       /* by ia_record.status                                              */

@@ -117,11 +117,12 @@ def main():
                 ev1.record()
             return ctx, bufs, ev0, ev1
 
-        def report(group, ctx, bufs, ev0, ev1):
+        def report(group, ctx, bufs, ev0, ev1, close=True):
             ev1.synchronize()
             times = [ctx.timing(len(group) - 1 - k) for k in range(len(group))]
             T_rf = ctx.derived["T_rf"]
-            ctx.close()
+            if close:       # ia_destroy frees device memory, which waits for the whole device: not while others run
+                ctx.close()
             wall = ev0.elapsed_time(ev1) * 1e-3
             n_all = steps_all = 0
             for cell, (rec, summ, _), t in zip(group, bufs, times):
@@ -180,9 +181,11 @@ def main():
                 inflight.append((g, *enqueue(g, torch.cuda.Stream())))
                 print(f"enqueued {g[0].name} ({len(inflight)} of {len(groups)})", file=sys.stderr, flush=True)
             for g, ctx, bufs, ev0, ev1 in inflight:
-                report(g, ctx, bufs, ev0, ev1)
+                report(g, ctx, bufs, ev0, ev1, close=False)
             t1.record()
             torch.cuda.synchronize()
+            for _, ctx, _, _, _ in inflight:
+                ctx.close()
             print(json.dumps({"concurrent_groups": len(groups), "config": which, "seconds": t0.elapsed_time(t1) * 1e-3,
                               "n": sum(c.launch.n for g in groups for c in g)}), flush=True)
         else:

@@ -427,9 +427,14 @@ def test_config1_subgrid_ensemble_and_regular_region(P):
     reg = (ref["n_coll"] == 1) & (rec["n_coll"] == 1) & (ref["status"] == 0)
     assert reg.sum() > 500
     same, e_t, e_dir, e_v, e_k = _compare_regular(rec[reg], ref[reg], "config1 regular region")
-    assert same.mean() >= 0.97
-    assert np.median(e_t[same]) <= 1e-8 and np.median(e_dir[same]) <= 1e-8
-    assert np.quantile(e_t[same], 0.99) <= 1e-5
+    # Bars = about three times what is measured (1 624 of 1 629 sequences identical; t_dwell 5e-10 / 8e-8 / 2e-7 median /
+    # 99 % / max; ke_ion 6e-8 / 1e-5 / 2e-4).  They sit above config 0's because the floor scales as (D_e/E) eps sqrt(N) on
+    # the outgoing energy (D_e/E = 6.7e5 here against 1e5) and ke_ion carries 2 pi t_dwell/T_rf = 280 rad of micromotion
+    # phase (R19); north_star's 1e-8 is held on config 0, and here by the medians of t_dwell and of the direction.
+    assert same.mean() >= 0.99
+    assert np.median(e_t[same]) <= 2e-9 and np.median(e_dir[same]) <= 1e-9
+    assert np.quantile(e_t[same], 0.99) <= 3e-7 and e_t[same].max() <= 1e-6
+    assert np.median(e_k[same]) <= 3e-7 and np.quantile(e_k[same], 0.99) <= 5e-5
     # chaotic trajectories agree as an ensemble, not one by one (R14); counts still have to add up
     assert int(summ["n_done"]) == cell.launch.n
     assert int(summ["n_complex"]) == int((rec["n_coll"] >= 2).sum())
@@ -470,8 +475,11 @@ def test_config1_full_grid_in_the_bench_configuration(P):
     reg = (ref["n_coll"] == 1) & (got["n_coll"] == 1) & (ref["status"] == 0)
     assert reg.sum() > 500
     same, e_t, e_dir, e_v, e_k = _compare_regular(got[reg], ref[reg], "config1 512x512 regular region")
-    assert same.mean() >= 0.97
-    assert np.median(e_t[same]) <= 1e-8 and np.median(e_dir[same]) <= 1e-8
+    # measured: 1 631 of 1 633 sequences identical; t_dwell 5e-10 / 6e-8 / 1e-7 (median / 99 % / max); ke_ion 6e-8 / 1e-5
+    assert same.mean() >= 0.99
+    assert np.median(e_t[same]) <= 2e-9 and np.median(e_dir[same]) <= 1e-9
+    assert np.quantile(e_t[same], 0.99) <= 3e-7 and e_t[same].max() <= 1e-6
+    assert np.median(e_k[same]) <= 3e-7 and np.quantile(e_k[same], 0.99) <= 5e-5
     # properties that hold at any size
     assert int(summ["n_done"]) == n and int(summ["n_status"].sum()) == n
     assert int(summ["n_complex"]) == int((rec["n_coll"] >= 2).sum())
@@ -553,8 +561,10 @@ def test_thermal_run_ensemble(P):
     reg = (ref["n_coll"] <= 1) & (rec["n_coll"] <= 1) & (ref["status"] == 0) & (rec["status"] == 0)
     assert reg.sum() > 1000 and (ref["n_coll"] == 0).sum() > 100            # many atoms never reach short range
     same, e_t, e_dir, e_v, e_k = _compare_regular(rec[reg], ref[reg], "thermal regular trajectories")
-    assert same.mean() >= 0.95
-    assert np.median(e_t[same]) <= 1e-8 and np.median(e_dir[same]) <= 1e-8
+    # measured: 3 788 of 3 789 sequences identical; t_dwell 6e-15 / 4e-8 (median / 99 %): most atoms pass at a distance
+    assert same.mean() >= 0.995
+    assert np.median(e_t[same]) <= 1e-10 and np.median(e_dir[same]) <= 1e-10
+    assert np.quantile(e_t[same], 0.99) <= 2e-7 and np.quantile(e_k[same], 0.99) <= 2e-6
     assert int(summ["n_done"]) == cell.launch.n
     assert int(summ["n_complex"]) == int((rec["n_coll"] >= 2).sum())
     assert np.array_equal(summ["hist_ncoll"], S.ncoll_bins(rec["n_coll"]).astype(np.uint64))
@@ -647,8 +657,11 @@ def test_deep_well_cell_ensemble(P):
     assert ok, detail
     reg = (ref["n_coll"] == 1) & (rec["n_coll"] == 1) & (ref["status"] == 0) & (rec["status"] == 0)
     same, e_t, e_dir, e_v, e_k = _compare_regular(rec[reg], ref[reg], "D_e = 100 K regular region")
+    # measured: 905 of 922 sequences identical; t_dwell 3e-7 / 2e-5 (median / 99 %), direction 7e-8 median: the floor
+    # (D_e/E) eps sqrt(N) = 3e7 x 1e-16 x 30 = 1e-7 of this cell, three hundred times config 0's
     assert reg.sum() > 500 and same.mean() >= 0.95
-    assert np.median(e_t[same]) <= 1e-5 and np.median(e_dir[same]) <= 1e-5
+    assert np.median(e_t[same]) <= 1e-6 and np.median(e_dir[same]) <= 3e-7
+    assert np.quantile(e_t[same], 0.99) <= 1e-4
     assert int(summ["n_done"]) == 2048 and rec["n_loc"].max() < 60
 
 
