@@ -303,7 +303,9 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
             const unsigned K = (G.mode == IA_IC_THERMAL) ? 111u : 59u;
             unsigned B = 1u;
             while (B < 8u && (B + 1u) * (B + 1u) * I <= K) ++B;
-            if ((unsigned)__popc(wm) < B && __any_sync(IA_FULL, mode != MODE_IDLE)) wm = 0u;
+            /* ... but not for longer than collecting B lanes should take (the rest of the warp may be long-lived) */
+            const bool overdue = iters - sh.last_fin[threadIdx.x] > 2u * B * I + IA_INNER;
+            if ((unsigned)__popc(wm) < B && !overdue && __any_sync(IA_FULL, mode != MODE_IDLE)) wm = 0u;
         }
         if (wm) {
             const int first = __ffs(wm) - 1;
