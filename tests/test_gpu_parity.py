@@ -846,6 +846,18 @@ def test_no_out_of_bounds_writes_guard_zones(P):
         _, sh = ctx.run_host(c1.launch)
         assert int(sh["n_done"]) == n
         ctx.debug_check()
+        # more submitted host runs than the ctx keeps summaries for (64): the 65th submit waits for the first 64 itself
+        small = replace(c1.launch, n=96)
+        many = [(torch.zeros(96 * 64, dtype=torch.uint8).pin_memory(), torch.zeros(1024, dtype=torch.uint8).pin_memory())
+                for _ in range(70)]
+        for rh, sm in many:
+            P.ia_submit_host(ctx.handle, P.make_launch(small), rh, sm)
+        ctx.wait()
+        first = many[0][0].numpy().view(P.RECORD_DTYPE)
+        for rh, sm in many:
+            assert int(sm.numpy().view(P.SUMMARY_DTYPE)[0]["n_done"]) == 96
+            _assert_records_identical(rh.numpy().view(P.RECORD_DTYPE), first)
+        ctx.debug_check()
     th = I.thermal("Rb87", 1.0, n=1000)
     th = replace(th, params=replace(th.params, t_max_rf=40.0))
     with P.Context(th.params) as ctx:
