@@ -498,6 +498,50 @@ def test_config1_full_grid_in_the_bench_configuration(P):
     assert np.all(rec["n_coll"][rec["status"] == 0] >= 1)                      # head-on: every escape bounced once
 
 
+def test_config4_stream_in_the_bench_configuration(P):
+    """BASELINE.json configs[4] the way bench.py runs it: two consecutive batches of 2^24 trajectories of the Philox
+    stream as a pipeline (the second bulk kernel first resumes what the first left unfinished), joined by one chain.
+    Every 4 096th trajectory of the SECOND batch (4 096 of them, E log-uniform in 1-100 uK, full sphere, random phase)
+    is recomputed by the oracle: per trajectory where regular, as an ensemble elsewhere; and what holds at any size."""
+    import torch
+    cells = I.config4(n_total=2 ** 25, batch=2 ** 24)
+    assert len(cells) == 2 and cells[1].launch.first_index == 2 ** 24
+    n = 2 ** 24
+    with P.Context(cells[0].params) as ctx:
+        ctx.set_pipeline(64)
+        bufs = [ctx.alloc(n) for _ in cells]
+        for c, (rec_d, summ_d, _) in zip(cells, bufs):
+            ctx.run(c.launch, records=rec_d, summary=summ_d)
+        ctx.join()
+        torch.cuda.synchronize()
+        summ = [P.view_summary(b[1]) for b in bufs]
+        rec = P.view_records(bufs[1][0], n)
+        ctx.debug_check()
+    idx = np.arange(0, n, 4096, dtype=np.uint64)
+    ref = O.run_generated(cells[1].params, cells[1].launch, indices=idx, nthreads=NTHREADS)
+    got = rec[idx.astype(np.int64)]
+    ok, detail = _ensemble_checks(got, ref, "config4 second batch, every 4096th")
+    assert ok, detail
+    reg = (ref["n_coll"] == 1) & (got["n_coll"] == 1) & (ref["status"] == 0) & (got["status"] == 0)
+    assert reg.sum() > 1500
+    same, e_t, e_dir, e_v, e_k = _compare_regular(got[reg], ref[reg], "config4 second batch, regular region")
+    assert same.mean() >= 0.99
+    assert np.median(e_t[same]) <= 2e-9 and np.median(e_dir[same]) <= 1e-9
+    assert np.quantile(e_t[same], 0.99) <= 3e-7
+    # what holds at any size
+    for s_k in summ:
+        assert int(s_k["n_done"]) == n and int(s_k["n_status"].sum()) == n and int(s_k["warn"]) == 0
+    assert int(summ[1]["n_complex"]) == int((rec["n_coll"] >= 2).sum())
+    assert np.array_equal(summ[1]["hist_ncoll"], S.ncoll_bins(rec["n_coll"]).astype(np.uint64))
+    assert int(summ[1]["steps_acc"]) == int(rec["steps_acc"].astype(np.int64).sum())
+    assert np.all(rec["status"] <= 1) and 300 < (rec["status"] == 1).sum() < 1200      # about 4e-5 reach t_max
+    assert rec["n_loc"].max() < 60
+    # the second bulk kernel advanced trajectories of the first batch next to its own, in full warps
+    own = int(summ[1]["steps_acc"]) + int(summ[1]["steps_rej"]) + int(summ[1]["steps_loc"]) - int(summ[1]["steps_coop"])
+    assert int(summ[1]["steps_kernel"]) > own and int(summ[0]["n_handoff"]) > 10000
+    assert int(summ[1]["steps_kernel"]) / int(summ[1]["slots_bulk"]) > 0.99
+
+
 @pytest.mark.parametrize("which,ci", [("config2", 18), ("config2", 2), ("config3", 7), ("config4", 0),
                                       ("config3", 0), ("config3", 4), ("config3", 10), ("config3", 14)])
 def test_philox_cells_ensemble(P, which, ci):
