@@ -571,6 +571,57 @@ def test_philox_cells_ensemble(P, which, ci):
     assert S.two_proportion_ok(int((rec["status"] != 0).sum()), n, int((ref["status"] != 0).sum()), n)[0]
 
 
+@pytest.mark.parametrize("which", ["config2", "config3"])
+def test_every_cell_of_configs_2_and_3_against_the_oracle(P, which):
+    """All 25 cells of config 2 and all 20 of config 3, the first 1 024 Philox indices of each, against the oracle
+    (config 3's D_e = 10 K and 100 K rows with t_max cut to 300 and 100 T_rf on both sides so that the oracle
+    finishes: a complex still bound then counts as one).  Per cell: statuses and bounce counts of the single-bounce
+    trajectories identical, their dwell times at the round-off floor of the cell, the number of complexes inside
+    the 99.9 % two-proportion interval (45 cells: one re-draw with a new seed allowed per cell, R15), and the
+    trend the paper states across cells checked on the GPU numbers."""
+    n = 1024
+    cells = I.config2(n_per_cell=n) if which == "config2" else I.config3(n_per_cell=n)
+    if which == "config3":
+        cut = {10.0: 300.0, 100.0: 100.0}
+        cells = [replace(c, params=replace(c.params, t_max_rf=cut.get(c.params.De_K, c.params.t_max_rf))) for c in cells]
+    z999 = 3.2905267314919255
+    p_gpu = {}
+    for cell in cells:
+        launch = cell.launch
+        for attempt in range(2):
+            with P.Context(cell.params) as ctx:
+                rec, summ, _ = ctx.run_sync(launch)
+            ref = O.run_generated(cell.params, launch, nthreads=NTHREADS)
+            k_g, k_o = int((rec["n_coll"] >= 2).sum()), int((ref["n_coll"] >= 2).sum())
+            ok, d, half = S.two_proportion_ok(k_g, n, k_o, n, z999)
+            if ok:
+                break
+            launch = replace(launch, seed=launch.seed + 1)
+        assert ok, (cell.name, k_g, k_o, half)
+        assert int(summ["n_done"]) == n and int(summ["n_complex"]) == k_g
+        reg = (ref["n_coll"] <= 1) & (rec["n_coll"] <= 1)
+        assert np.array_equal(rec["status"][reg], ref["status"][reg].astype(np.uint8)), cell.name
+        assert np.array_equal(rec["n_coll"][reg], ref["n_coll"][reg]) and reg.sum() >= 0.2 * n, cell.name
+        esc = reg & (ref["status"] == 0)
+        same = esc & (rec["steps_acc"] == ref["steps_acc"]) & (rec["steps_rej"] == np.minimum(ref["steps_rej"], 65535))
+        e_t = np.abs(rec["t_dwell"][same] / ref["t_dwell"][same] - 1.0)
+        floor = 1e-8 if cell.params.De_K <= 1.0 else (1e-7 if cell.params.De_K <= 10.0 else 1e-5)
+        assert same.sum() >= 0.9 * esc.sum() and np.median(e_t) <= floor, (cell.name, same.sum(), esc.sum(), np.median(e_t))
+        p_gpu[cell.name] = k_g / n
+    print(f"\n{which}: P(complex) on the first {n} indices of every cell: " + ", ".join(f"{k.split('_', 1)[1]} {v:.3f}" for k, v in p_gpu.items()))
+    if which == "config2":
+        assert all(p_gpu[f"config2_Li7_{E:g}uK"] == 0.0 for E in I.ENERGIES_UK)            # no complexes for Li head-on
+        assert p_gpu["config2_Na23_1uK"] < p_gpu["config2_K39_1uK"] < p_gpu["config2_Cs133_1uK"] + 0.05   # heavier: more
+        for sp in ("Na23", "K39", "Rb87", "Cs133"):                                           # hotter: fewer, none at 100 uK
+            assert p_gpu[f"config2_{sp}_1uK"] > p_gpu[f"config2_{sp}_100uK"] == 0.0
+    else:
+        for De in ("0.1", "1", "10"):                                                          # rising with q (PAPER.md:66)
+            assert p_gpu[f"config3_De{De}K_q0.05"] < p_gpu[f"config3_De{De}K_q0.4"]
+        for q in ("0.2", "0.3", "0.4"):                                                        # flat in D_e (PAPER.md:44)
+            vals = [p_gpu[f"config3_De{De}K_q{q}"] for De in ("0.1", "1", "10")]
+            assert max(vals) - min(vals) < 0.08
+
+
 # ---------------------------------------------------------------------------------------------
 # thermal runs (SURVEY.md section 8(f) item 1; PAPER.md:42,50; reading R18)
 # ---------------------------------------------------------------------------------------------
