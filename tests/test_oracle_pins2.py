@@ -454,3 +454,70 @@ def test_roundoff_floor_of_the_adaptive_path_oracle_against_itself(tmp_path):
           f"ke_ion max {e_k.max():.2e} median {np.median(e_k):.2e}; va_f max {e_v.max():.2e} median {np.median(e_v):.2e}")
     assert e_t.max() < 2e-9 and e_v.max() < 5e-9                       # below the 1e-8 of north_star
     assert 1e-8 < e_k.max() < 1e-7 and 3e-10 < np.median(e_k) < 3e-9   # the floor of ke_ion is NOT below it
+
+
+# --------------------------------------------------------------------------------------------
+# the oracle under AddressSanitizer and UndefinedBehaviorSanitizer
+# --------------------------------------------------------------------------------------------
+_ASAN_DRIVER = r"""
+#include <cstdio>
+#include <cstring>
+#include <vector>
+#include "ia_oracle.h"
+int main() {
+    oracle_params p;
+    std::memset(&p, 0, sizeof(p));
+    p.m_ion_u = 173.94; p.m_atom_u = 86.909; p.alpha_au = 319.2;
+    p.a[0] = -0.0005; p.a[1] = -0.0005; p.a[2] = 0.001; p.q[0] = 0.1; p.q[1] = -0.1; p.q[2] = 0.0;
+    p.omega_rf_au = 3.0396596921148e-10; p.De_K = 1.0; p.r0_a0 = 5000.0; p.rtol = 1e-10; p.atol = 1e-12;
+    p.t_max_rf = 60.0; p.h_max_rf = 0.25; p.r_coll_a0 = 500.0; p.max_steps = 1ull << 31;
+    unsigned long long done = 0, complexes = 0;
+    for (int mode = 1; mode <= 3; ++mode) {           /* GRID, PHILOX, THERMAL */
+        oracle_gen g;
+        std::memset(&g, 0, sizeof(g));
+        g.mode = mode; g.domain = mode == 1 ? 0 : 1; g.phase_mode = mode == 1 ? 0 : 1; g.n_theta = 7; g.n_phi = 9;
+        g.E_min_uK = 1.5; g.E_max_uK = mode == 2 ? 100.0 : 1.5; g.seed = 12345; g.cell = 7; g.first_index = mode == 2 ? (1ull << 33) - 5 : 0;
+        g.T_atom_uK = 3.0; g.T_ion_uK = 10.0;
+        const uint64_t n = 63;
+        std::vector<oracle_outcome> out(n);
+        if (oracle_run_generated(&p, &g, nullptr, 0, n, out.data(), 3) != 0) return 2;
+        for (const auto &o : out) { ++done; complexes += o.n_coll >= 2; if (o.status < 0 || o.status > 4) return 3; }
+    }
+    /* trace and path buffers at their exact sizes */
+    double y0[12], ph, E;
+    oracle_gen g; std::memset(&g, 0, sizeof(g)); g.mode = 1; g.n_theta = 4; g.n_phi = 4; g.E_min_uK = g.E_max_uK = 1.5;
+    if (oracle_generate(&p, &g, 5, y0, &ph, &E) != 0) return 4;
+    std::vector<double> states(13 * 41);
+    oracle_trace(&p, y0, ph, 1e8, 40, states.data());
+    std::vector<double> path(13 * 100);
+    oracle_outcome o; uint64_t len = 0;
+    oracle_run(&p, y0, ph, &o, path.data(), 100, &len);
+    if (len > 100) return 5;
+    std::printf("%llu trajectories, %llu complexes\n", done, complexes);
+    return 0;
+}
+"""
+
+
+def test_oracle_is_clean_under_asan_and_ubsan(tmp_path):
+    """The oracle's source compiled with -fsanitize=address,undefined (no recovery) into a small driver that runs all
+    three generators (ragged counts, an index that carries into the second counter word, three worker threads),
+    a fixed-step trace and a path dump into buffers of exactly the documented sizes: exits 0 with no report."""
+    import shutil
+    if shutil.which("g++") is None:
+        pytest.skip("g++ not on PATH")
+    odir = os.path.dirname(O.__file__)
+    src = tmp_path / "driver.cpp"
+    src.write_text(_ASAN_DRIVER)
+    exe = tmp_path / "driver"
+    flags = ["-std=c++17", "-O1", "-g", "-ffp-contract=off", "-pthread", "-fsanitize=address,undefined",
+             "-fno-sanitize-recover=all", "-fno-omit-frame-pointer"]
+    r = subprocess.run(["g++", *flags, "-I", odir, "-o", str(exe), str(src), os.path.join(odir, "ia_oracle.cpp")],
+                       capture_output=True, text=True)
+    if r.returncode != 0 and "asan" in (r.stderr or "").lower():
+        pytest.skip("sanitizer runtime not installed")
+    assert r.returncode == 0, r.stderr[-2000:]
+    run = subprocess.run([str(exe)], capture_output=True, text=True, timeout=300,
+                         env={**os.environ, "ASAN_OPTIONS": "detect_leaks=1:abort_on_error=0"})
+    assert run.returncode == 0, (run.stdout[-500:], run.stderr[-3000:])
+    assert "189 trajectories" in run.stdout and "ERROR" not in run.stderr
