@@ -287,6 +287,11 @@ int ia_get_last_timing(ia_ctx *ctx, double *bulk_ms, double *coop_ms);
  * tflops = 2 * DFMA/s / 1e12; elapsed_ms = CUDA-event time of the timed launch. */
 int ia_fp64_peak(int cuda_device, double target_ms, double *tflops, double *elapsed_ms);
 
+/* Latency microbenchmark (the floor of the straggler chain): one warp, one dependent chain.
+ * cycles_dfma = SM cycles per dependent DFMA; cycles_rcp_add = SM cycles per reciprocal as the right-hand side
+ * computes it (MUFU.RCP64H and three dependent DFMA) followed by one dependent DADD.  Host pointers. */
+int ia_fp64_latency(int cuda_device, double *cycles_dfma, double *cycles_rcp_add);
+
 /* Debugging aid (compute-sanitizer is not available on every machine): every device buffer a ctx owns -- hand-over
  * queues, counters, summaries and records staged for the host entry points, the late-record list -- is allocated
  * with 4 KiB guard zones of a known byte pattern on either side, and the kernels refuse to write a queue or list

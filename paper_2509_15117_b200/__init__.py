@@ -32,7 +32,7 @@ IA_STRAGGLER_LEVELS = 12
 # every symbol include/ia.h declares (tests/test_cabi.py checks the library exports each of them)
 EXPORTS = ("ia_create", "ia_run", "ia_run_host", "ia_generate", "ia_step_map", "ia_trace", "ia_get_derived",
            "ia_get_kernel_info", "ia_set_handoff", "ia_set_chain", "ia_get_last_timing", "ia_get_timing", "ia_set_pipeline", "ia_join",
-           "ia_submit_host", "ia_sync", "ia_wait", "ia_debug_check", "ia_fp64_peak", "ia_destroy", "ia_strerror", "ia_last_error")
+           "ia_submit_host", "ia_sync", "ia_wait", "ia_debug_check", "ia_fp64_peak", "ia_fp64_latency", "ia_destroy", "ia_strerror", "ia_last_error")
 
 
 class IaError(RuntimeError):
@@ -119,6 +119,7 @@ def load() -> C.CDLL:
     L.ia_sync.argtypes = [vp]
     L.ia_debug_check.argtypes = [vp]
     L.ia_fp64_peak.argtypes = [C.c_int, C.c_double, dp, dp]
+    L.ia_fp64_latency.argtypes = [C.c_int, dp, dp]
     L.ia_destroy.argtypes = [vp]
     L.ia_strerror.argtypes = [C.c_int]
     L.ia_strerror.restype = C.c_char_p
@@ -304,6 +305,13 @@ def ia_fp64_peak(device: int = 0, target_ms: float = 200.0) -> dict:
     t, ms = C.c_double(), C.c_double()
     _check(load().ia_fp64_peak(int(device), float(target_ms), C.byref(t), C.byref(ms)))
     return {"tflops": t.value, "elapsed_ms": ms.value}
+
+
+def ia_fp64_latency(device: int = 0) -> dict:
+    """SM cycles per dependent DFMA and per reciprocal (MUFU.RCP64H + 3 DFMA) + DADD, one warp alone."""
+    a, b = C.c_double(), C.c_double()
+    _check(load().ia_fp64_latency(int(device), C.byref(a), C.byref(b)))
+    return {"cycles_dfma": a.value, "cycles_rcp_add": b.value}
 
 
 # ---- convenience wrapper ---------------------------------------------------------------------------

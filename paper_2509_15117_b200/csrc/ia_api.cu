@@ -886,4 +886,13 @@ int ia_fp64_peak(int cuda_device, double target_ms, double *tflops, double *elap
     return ia_run_fp64_peak(cuda_device, target_ms, tflops, elapsed_ms) == cudaSuccess ? IA_OK : IA_ECUDA;
 }
 
+int ia_fp64_latency(int cuda_device, double *cycles_dfma, double *cycles_rcp_add) {
+    if (!cycles_dfma || !cycles_rcp_add) return IA_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || cuda_device < 0 || cuda_device >= ndev) return IA_EDEVICE;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, cuda_device) != cudaSuccess || prop.major != 10) return IA_EDEVICE;
+    return ia_run_fp64_latency(cuda_device, cycles_dfma, cycles_rcp_add) == cudaSuccess ? IA_OK : IA_ECUDA;
+}
+
 } // extern "C"

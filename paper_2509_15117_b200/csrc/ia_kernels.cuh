@@ -98,3 +98,5 @@ cudaError_t ia_launch_trace(int variant, const IaParams &P, IaY12 y0, double pha
 
 /* DFMA peak microbenchmark */
 cudaError_t ia_run_fp64_peak(int device, double target_ms, double *tflops, double *elapsed_ms);
+/* latency of a dependent DFMA, and of the reciprocal (MUFU.RCP64H + 3 DFMA) plus one DADD, in SM cycles */
+cudaError_t ia_run_fp64_latency(int device, double *cycles_dfma, double *cycles_rcp_add);

@@ -68,3 +68,47 @@ cudaError_t ia_run_fp64_peak(int device, double target_ms, double *tflops, doubl
     cudaFree(sink);
     return e;
 }
+
+/* Latency of DEPENDENT FP64 operations, in SM cycles: one warp, one chain.  What bounds the step of a lone warp
+ * (the end of a stream) is the length of the step's dependent chain times this. */
+__global__ void ia_fp64_latency_kernel(double *out, unsigned n, double a, double b) {
+    double x = 0.5 + 1e-3 * (double)threadIdx.x;
+    long long t0 = clock64();
+#pragma unroll 1
+    for (unsigned it = 0; it < n; ++it) {
+#pragma unroll
+        for (int u = 0; u < 64; ++u) x = fma(x, a, b);
+    }
+    long long t1 = clock64();
+    double y = 1.5 + 1e-3 * (double)threadIdx.x;
+#pragma unroll 1
+    for (unsigned it = 0; it < n; ++it) {
+#pragma unroll
+        for (int u = 0; u < 16; ++u) y = ia_rcp(y) + a; /* MUFU.RCP64H + 3 DFMA, then one DADD */
+    }
+    long long t2 = clock64();
+    if (threadIdx.x == 0) {
+        out[0] = (double)(t1 - t0) / (64.0 * n);
+        out[1] = (double)(t2 - t1) / (16.0 * n);
+        out[2] = x + y;
+    }
+}
+
+cudaError_t ia_run_fp64_latency(int device, double *cycles_dfma, double *cycles_rcp_add) {
+    cudaError_t e = cudaSetDevice(device);
+    if (e != cudaSuccess) return e;
+    double *out = nullptr;
+    e = cudaMalloc(&out, 3 * sizeof(double));
+    if (e != cudaSuccess) return e;
+    double h[3] = {0, 0, 0};
+    for (int rep = 0; rep < 2 && e == cudaSuccess; ++rep) { /* the second launch is the measurement */
+        ia_fp64_latency_kernel<<<1, 32>>>(out, 2000u, 0.999999, 1e-7);
+        e = cudaMemcpy(h, out, sizeof(h), cudaMemcpyDeviceToHost);
+    }
+    cudaFree(out);
+    if (e == cudaSuccess) {
+        *cycles_dfma = h[0];
+        *cycles_rcp_add = h[1];
+    }
+    return e;
+}

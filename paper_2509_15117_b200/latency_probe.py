@@ -40,6 +40,9 @@ def main():
         steps = int(steps_all[j])
         print(f"{len(bound)} trajectories of the 128 x 128 map still bound at {t_max:g} T_rf; replicating number {j}: "
               f"{steps} attempted steps, {rec['n_coll'][j]} bounces")
+        lat = P.ia_fp64_latency(0)
+        print(f"dependent DFMA: {lat['cycles_dfma']:.2f} SM cycles; reciprocal (MUFU.RCP64H + 3 DFMA) + DADD: "
+              f"{lat['cycles_rcp_add']:.2f} cycles\n")
         print("| layout | warps per sub-partition | trajectories | ms | us per step | 1e9 steps/s |")
         print("|---|---|---|---|---|---|")
         for path, name, per_warp in ((P.IA_PATH_COOP_ONLY, "cooperative (3 lanes)", 10), (P.IA_PATH_BULK_ONLY, "bulk (1 lane)", 32)):
