@@ -37,11 +37,11 @@ import numpy as np  # noqa: E402
 import ia_inputs as I  # noqa: E402
 
 METRIC = "trajectories/s"
-# Algorithmic FP64 flops per ATTEMPTED RK step (FMA = 2), counted from the formulas of the
-# Nystrom-collapsed DP5(4) step in DESIGN.md section "Roofline": coefficient products 35, five cosines 135,
-# stage sums 300, six accelerations 234, d.w 8, error sums 120, norm cross-products 22,
-# controller / time keeping 32.
-FLOP_PER_STEP = 886.0
+# FP64 flops per ATTEMPTED RK step (FMA = 2) of the Nystrom-collapsed DP5(4) step as the kernels compute it
+# (DESIGN.md section "Roofline"): 345 FMA + 144 products + 33 sums = 867.  It is the count of the formulas AND the
+# count ncu reads off the bulk kernel (sass__inst_executed_per_opcode per warp and step: DFMA 345.0, DMUL 143.6,
+# DADD 33.0; compares are not counted).  Round 1's step needed 886: the error norm and the controller have shed 19.
+FLOP_PER_STEP = 867.0
 ORACLE_SAMPLE_EVERY = 8   # oracle legs on a GRID workload: every 8th grid point in theta and phi (64x64 = 4,096)
 ORACLE_SAMPLE_PHILOX = 8192   # ... on a Philox stream: its first 8,192 indices (reference arm, per step)
 ORACLE_SAMPLE_BASELINE = 32768  # ... and for the one-shot cpu_baseline of our arm
