@@ -30,6 +30,7 @@
  */
 #ifndef IA_H
 #define IA_H
+#include <stddef.h>
 #include <stdint.h>
 
 #ifdef __cplusplus
@@ -299,6 +300,51 @@ int ia_fp64_latency(int cuda_device, double *cycles_dfma, double *cycles_rcp_add
  * work in flight has finished, then verifies every guard zone, the fault word and the device-side counts
  * (IA_ECUDA / IA_EINVAL with the finding in ia_last_error). */
 int ia_debug_check(ia_ctx *ctx);
+
+/* ia_run_static -- one launch of the production kernel pair for callers that must not allocate device memory.
+ *
+ * Who needs it.  Every other way into this library goes through ia_create, which takes its work counters and
+ * hand-over queues from cudaMalloc.  Some hosts of this code cannot do that: a plug-in running inside an application
+ * whose own pool allocator has already claimed the GPU's memory (a cudaMalloc next to it fails, or fragments the
+ * pool), and a control loop that launches between other streams' work and cannot afford the device-wide
+ * synchronisation cudaMalloc / cudaFree imply.  For them this call needs no ctx and calls no cudaMalloc, cudaFree,
+ * cudaMallocHost or any other allocating routine, on any call: its scratch (six counter words and a hand-over queue
+ * of IA_STATIC_MAX_N entries of 256 bytes, 4 MiB + 256 bytes in all) is a static array inside the library's device
+ * image.  Every GPU the process loads the library on carries those 4 MiB from the moment the module is loaded until
+ * the process exits, used or not; that is the price, and why the limit is modest.
+ *
+ * What it computes.  Exactly what ia_create + ia_run(IA_PATH_AUTO, no pipeline) compute for the same cell and
+ * launch: the bulk kernel (one lane per trajectory) propagates, hands what still runs in a drained warp to the
+ * queue, and one launch of the cooperative kernel (three lanes per trajectory) finishes it.  Records are
+ * bit-identical to ia_run's; the summary is accumulated into, as there (zero it first, on `cuda_stream`).
+ * species / trap / De_K / r0_a0 / tol are ia_create's arguments (HOST pointers, tol may be NULL), launch and
+ * outputs are ia_run's (the structs are HOST memory, every pointer inside them a DEVICE pointer on `cuda_device`:
+ * the caller still owns and passes all inputs and outputs).  launch->path must be IA_PATH_AUTO.  Enqueues a
+ * 256-byte memset and two kernels on `cuda_stream` and returns without synchronising; makes `cuda_device` the
+ * calling thread's current device.  n = 0 is valid and launches nothing.
+ *
+ * Limit.  launch->n <= IA_STATIC_MAX_N (the queue holds one entry per trajectory of the launch).  A larger launch
+ * is refused with IA_EINVAL before anything is enqueued, and the text says so; cut it into several calls on one
+ * stream (first_index advances), or use ia_create / ia_run.
+ *
+ * First call on a device.  It looks up the device address of the static array and the launch geometry of the two
+ * kernels (which makes the CUDA runtime load the library's kernels onto that device) and keeps both for the
+ * process's lifetime; later calls on that device only launch.  Make that first call during start-up, outside any
+ * stream capture and before the phase in which allocation is forbidden.
+ *
+ * Sharing.  All calls on a device use the same array.  The call clears the counter words it needs on
+ * `cuda_stream` before its kernels; the queue keeps whatever the previous call left and is never read beyond what
+ * the current call wrote.  Two calls whose kernels can overlap on the GPU -- different streams without an event
+ * between them, or two host threads -- race on the counters and corrupt each other's results: keep all calls of a
+ * device on one stream, or order them with events.  The host side of the call is thread-safe.
+ *
+ * Errors.  IA_EINVAL / IA_EDEVICE / IA_ECUDA as elsewhere; errbuf (HOST, may be NULL) receives at most
+ * errbuf_len - 1 characters of explanation and a terminating NUL -- "" on plain success, the PAPER.md:28
+ * asymptotic-start warning when that applies.  On failure nothing was enqueued. */
+#define IA_STATIC_MAX_N 16384
+int ia_run_static(const ia_species *species, const ia_trap *trap, double De_K, double r0_a0, const ia_tol *tol,
+                  int cuda_device, const ia_launch *launch, const ia_outputs *outputs, void *cuda_stream,
+                  char *errbuf, size_t errbuf_len);
 
 int ia_destroy(ia_ctx *ctx);
 const char *ia_strerror(int code);

@@ -28,11 +28,12 @@ IA_ARITH_NOFMA, IA_ARITH_FMA, IA_ARITH_FMA_COOP = 0, 1, 2
 IA_HIST_BINS = 32
 IA_LIFE_BINS = 64
 IA_STRAGGLER_LEVELS = 12
+IA_STATIC_MAX_N = 16384   # most trajectories one ia_run_static call takes (include/ia.h)
 
 # every symbol include/ia.h declares (tests/test_cabi.py checks the library exports each of them)
 EXPORTS = ("ia_create", "ia_run", "ia_run_host", "ia_generate", "ia_step_map", "ia_trace", "ia_get_derived",
            "ia_get_kernel_info", "ia_set_handoff", "ia_set_chain", "ia_get_last_timing", "ia_get_timing", "ia_set_pipeline", "ia_join",
-           "ia_submit_host", "ia_sync", "ia_wait", "ia_debug_check", "ia_fp64_peak", "ia_fp64_latency", "ia_destroy", "ia_strerror", "ia_last_error")
+           "ia_submit_host", "ia_sync", "ia_wait", "ia_debug_check", "ia_fp64_peak", "ia_fp64_latency", "ia_run_static", "ia_destroy", "ia_strerror", "ia_last_error")
 
 
 class IaError(RuntimeError):
@@ -120,6 +121,8 @@ def load() -> C.CDLL:
     L.ia_debug_check.argtypes = [vp]
     L.ia_fp64_peak.argtypes = [C.c_int, C.c_double, dp, dp]
     L.ia_fp64_latency.argtypes = [C.c_int, dp, dp]
+    L.ia_run_static.argtypes = [C.POINTER(ia_species), C.POINTER(ia_trap), C.c_double, C.c_double, C.POINTER(ia_tol),
+                                C.c_int, C.POINTER(ia_launch), C.POINTER(ia_outputs), vp, C.c_char_p, C.c_size_t]
     L.ia_destroy.argtypes = [vp]
     L.ia_strerror.argtypes = [C.c_int]
     L.ia_strerror.restype = C.c_char_p
@@ -298,6 +301,34 @@ def ia_sync(handle) -> None:
 def ia_debug_check(handle) -> None:
     """Verifies the guard zones around every ctx-owned device buffer and the kernels' fault word; raises on a finding."""
     _check(load().ia_debug_check(handle), handle)
+
+
+def ia_run_static(params, launch: ia_launch, records=None, summary=None, ic_dump=None, device: int = 0,
+                  stream=None) -> str:
+    """The production kernel pair without a ctx and without any device allocation inside the library, for hosts
+    that cannot call cudaMalloc (a plug-in next to an application whose pool already owns the GPU's memory; a loop
+    that cannot take cudaMalloc's device-wide synchronisation): the counters and the hand-over queue live in a
+    static 4 MiB array of the library's device image.  At most IA_STATIC_MAX_N trajectories per call; calls that
+    may overlap on the GPU race (keep them on one stream).  The first call on a device also looks up that array's
+    address and loads the kernels: make it at start-up.  Same buffers as ia_run (device tensors, the summary is
+    accumulated into), same results bit for bit.  Asynchronous; returns the warning text ("" if none)."""
+    sp = ia_species(params.m_ion_u, params.m_atom_u, params.alpha_au)
+    tr = ia_trap((C.c_double * 3)(*params.a), (C.c_double * 3)(*params.q), params.omega_rf_au)
+    tol = ia_tol(params.rtol, params.atol, params.t_max_rf, params.h_max_rf, params.r_coll_a0, int(params.max_steps))
+    out = ia_outputs(_ptr(records), _ptr(summary), _ptr(ic_dump))
+    err = C.create_string_buffer(512)
+    L = load()
+    # torch's current stream is looked up only where there is a device: without one the library itself answers
+    # (IA_EINVAL for a bad argument, IA_EDEVICE otherwise)
+    st = stream or None
+    if not isinstance(stream, int):
+        import torch
+        st = _stream_handle(stream) if (stream is not None or torch.cuda.is_available()) else None
+    rc = L.ia_run_static(C.byref(sp), C.byref(tr), float(params.De_K), float(params.r0_a0), C.byref(tol), int(device),
+                         C.byref(launch), C.byref(out), st, err, len(err))
+    if rc != IA_OK:
+        raise IaError(rc, ia_strerror(rc) + ": " + err.value.decode())
+    return err.value.decode()
 
 
 def ia_fp64_peak(device: int = 0, target_ms: float = 200.0) -> dict:

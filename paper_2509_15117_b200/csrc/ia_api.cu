@@ -896,3 +896,234 @@ int ia_fp64_latency(int cuda_device, double *cycles_dfma, double *cycles_rcp_add
 }
 
 } // extern "C"
+
+/* ---- ia_run_static: the production kernel pair with every byte of scratch in static device memory ------------------
+ *
+ * For callers that may not allocate (include/ia.h says who and why).  Nothing below calls cudaMalloc, cudaFree,
+ * cudaMallocHost, cudaEventCreate or cudaStreamCreate; the only CUDA calls after the one-time set-up of a device are
+ * cudaSetDevice, one cudaMemsetAsync and two kernel launches. */
+
+#include <mutex>
+
+/* The scratch ia_create would have taken from cudaMalloc, for one launch of at most IA_STATIC_MAX_N trajectories:
+ *   words[0] work counter of the bulk kernel        words[3] fault word (queue overflow; cannot happen: n <= capacity)
+ *   words[1] length of the bulk kernel's input      words[4] late-list length (there is no late list: stays 0)
+ *            queue (there is none: stays 0)         words[5] work counter of the cooperative kernel
+ *   words[2] trajectories handed over = length of the cooperative kernel's input queue
+ *   q[]      the hand-over queue, one entry per trajectory of the launch at most
+ * The words are cleared at the start of every call; the queue is not (entries are written before they are read). */
+#define IA_STATIC_WORDS 32
+struct IaStaticScratch {
+    unsigned long long words[IA_STATIC_WORDS]; /* 256 bytes: the queue behind it stays 256-byte aligned */
+    IaHand q[IA_STATIC_MAX_N];
+};
+static_assert(sizeof(IaStaticScratch) == 256 + (size_t)IA_STATIC_MAX_N * 256, "4 MiB + 256 bytes of static scratch");
+
+/* File-scope device array: part of the library's device image on every GPU that loads it, until the process exits.
+ * In HOST code this name is only a handle for the runtime -- never a device address: it is handed to nothing but
+ * cudaGetSymbolAddress (static_device_setup), and the kernels get the pointer that call returns. */
+static __device__ __align__(256) unsigned char ia_static_scratch[sizeof(IaStaticScratch)];
+
+#define IA_STATIC_MAX_DEV 64
+struct IaStaticDev {
+    bool ready = false;
+    IaStaticScratch *scratch = nullptr; /* device address of ia_static_scratch on this device */
+    int n_sm = 0;
+    IaKernelInfo kinfo[2]; /* 0 bulk, 1 cooperative */
+};
+static IaStaticDev g_static_dev[IA_STATIC_MAX_DEV];
+static std::mutex g_static_mutex;
+
+static int static_fail(char *errbuf, size_t errbuf_len, int code, const char *text) {
+    if (errbuf && errbuf_len > 0) std::snprintf(errbuf, errbuf_len, "%s", text);
+    return code;
+}
+
+/* Once per device, with that device current: the device address of the static array and the launch geometry of
+ * the two persistent kernels.  Both are kept for the lifetime of the process. */
+static int static_device_setup(int dev, const IaStaticDev **out, char *errbuf, size_t errbuf_len) {
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    IaStaticDev &D = g_static_dev[dev];
+    if (!D.ready) {
+        int major = 0, n_sm = 0;
+        cudaError_t e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess || major != 10)
+            return static_fail(errbuf, errbuf_len, IA_EDEVICE, "ia_run_static: the device is not compute capability 10.x");
+        void *p = nullptr;
+        e = cudaGetSymbolAddress(&p, ia_static_scratch);
+        if (e != cudaSuccess || p == nullptr) {
+            char msg[200];
+            std::snprintf(msg, sizeof(msg), "ia_run_static: cudaGetSymbolAddress(static scratch): %s",
+                          e != cudaSuccess ? cudaGetErrorString(e) : "NULL address");
+            return static_fail(errbuf, errbuf_len, IA_ECUDA, msg);
+        }
+        IaStaticDev T;
+        for (int k = 0; k < 2 && e == cudaSuccess; ++k)
+            e = ia_persistent_info(k == 0 ? 1 : 3, &T.kinfo[k].blocks_per_sm, &T.kinfo[k].threads_per_block,
+                                   &T.kinfo[k].regs, &T.kinfo[k].local_bytes);
+        if (e != cudaSuccess || T.kinfo[0].blocks_per_sm < 1 || T.kinfo[1].blocks_per_sm < 1) {
+            char msg[200];
+            std::snprintf(msg, sizeof(msg), "ia_run_static: kernel attributes: %s", cudaGetErrorString(e));
+            return static_fail(errbuf, errbuf_len, IA_ECUDA, msg);
+        }
+        T.scratch = (IaStaticScratch *)p;
+        T.n_sm = n_sm;
+        T.ready = true;
+        D = T;
+    }
+    *out = &D;
+    return IA_OK;
+}
+
+/* a1 for a caller without a ctx: the checks and the derived constants of ia_create (BASELINE.json
+ * north_star), written into a host-only ia_ctx that owns no CUDA resource */
+static int prepare_cell(ia_ctx *c, const ia_species *sp, const ia_trap *tr, double De_K, double r0_a0, const ia_tol *tol) {
+    ia_tol T;
+    std::memset(&T, 0, sizeof(T));
+    if (tol) T = *tol;
+    if (T.rtol == 0.0) T.rtol = 1e-10;
+    if (T.atol == 0.0) T.atol = 1e-12;
+    if (T.t_max_rf == 0.0) T.t_max_rf = 1e4;
+    if (T.h_max_rf == 0.0) T.h_max_rf = 0.25;
+    if (T.r_coll_a0 == 0.0) T.r_coll_a0 = 500.0;
+    if (T.max_steps == 0) T.max_steps = 1ull << 31;
+    auto pos = [](double v) { return std::isfinite(v) && v > 0.0; };
+    if (!pos(sp->m_ion_u) || !pos(sp->m_atom_u) || !pos(sp->alpha_au) || !pos(De_K) || !pos(r0_a0) ||
+        !pos(tr->omega_rf_au))
+        return IA_EINVAL;
+    for (int k = 0; k < 3; ++k)
+        if (!std::isfinite(tr->a[k]) || !std::isfinite(tr->q[k])) return IA_EINVAL;
+    if (!(T.rtol >= 1e-13 && T.rtol <= 1e-3) || !pos(T.atol) || !pos(T.t_max_rf) ||
+        !(T.h_max_rf > 0.0 && T.h_max_rf <= 0.25) || !pos(T.r_coll_a0) || T.max_steps > (1ull << 32) - 1)
+        return IA_EINVAL;
+    IaParams &P = c->P;
+    std::memset(&P, 0, sizeof(P));
+    P.m_i = sp->m_ion_u * ME_PER_U;
+    P.m_a = sp->m_atom_u * ME_PER_U;
+    P.inv_m_a = 1.0 / P.m_a;
+    P.neg_inv_m_i = -1.0 / P.m_i;
+    P.C4 = sp->alpha_au / 2.0;
+    P.De = De_K * KB_EH_PER_K;
+    P.C8 = P.C4 * P.C4 / (4.0 * P.De);
+    P.r_e = std::pow(2.0 * P.C8 / P.C4, 0.25);
+    P.c8x8 = 8.0 * P.C8;
+    P.neg_c4x4 = -4.0 * P.C4;
+    P.c8_a = P.c8x8 / P.m_a;
+    P.c4_a = P.neg_c4x4 / P.m_a;
+    P.c8_i = -P.c8x8 / P.m_i;
+    P.c4_i = -P.neg_c4x4 / P.m_i;
+    P.omega = tr->omega_rf_au;
+    P.T_rf = 2.0 * PI / P.omega;
+    for (int k = 0; k < 3; ++k) {
+        P.ka[k] = -tr->a[k] * (P.omega * P.omega / 4.0);
+        P.kq[k] = -2.0 * tr->q[k] * (P.omega * P.omega / 4.0);
+    }
+    c->w_harm = std::fabs(tr->q[0]) * P.omega / std::pow(2.0, 1.5);
+    P.rtol = T.rtol;
+    P.atol = T.atol;
+    P.thr = T.atol / T.rtol;
+    P.h_max = T.h_max_rf * P.T_rf;
+    P.h_min = std::ldexp(P.T_rf, -40);
+    P.t_max_rf = T.t_max_rf;
+    P.t_max = T.t_max_rf * P.T_rf;
+    P.h0_scale = 0.8 * std::pow(T.rtol, 0.2);
+    P.r0 = r0_a0;
+    P.r0sq = r0_a0 * r0_a0;
+    P.r_coll = T.r_coll_a0;
+    P.rcsq = T.r_coll_a0 * T.r_coll_a0;
+    P.loc_tol = 1e-13 * P.r0sq;
+    P.max_steps = T.max_steps;
+    P.n_near = T.t_max_rf > 2.0 ? (unsigned)std::floor(std::fmin(T.t_max_rf - 2.0, 4294967295.0)) : 0u;
+    const double d[16] = {P.m_i, P.m_a, P.C4, P.C8, P.De, P.r_e, P.omega, P.T_rf,
+                          P.thr, P.h_max, P.h_min, P.t_max, P.r0, P.r_coll, P.rtol, P.atol};
+    std::memcpy(c->derived, d, sizeof(d));
+    return IA_OK;
+}
+
+extern "C" int ia_run_static(const ia_species *species, const ia_trap *trap, double De_K, double r0_a0,
+                             const ia_tol *tol, int cuda_device, const ia_launch *launch, const ia_outputs *outputs,
+                             void *cuda_stream, char *errbuf, size_t errbuf_len) {
+    if (errbuf && errbuf_len > 0) errbuf[0] = '\0';
+    if (!species || !trap || !launch || !outputs)
+        return static_fail(errbuf, errbuf_len, IA_EINVAL, "ia_run_static: species, trap, launch or outputs is NULL");
+    /* the size limit first: it depends on nothing but the argument */
+    if (launch->n > (uint64_t)IA_STATIC_MAX_N) {
+        char msg[256];
+        std::snprintf(msg, sizeof(msg),
+                      "ia_run_static: launch.n = %llu exceeds IA_STATIC_MAX_N = %d, the capacity of the hand-over queue in "
+                      "static device memory; cut the launch into several calls on one stream or use ia_create / ia_run",
+                      (unsigned long long)launch->n, IA_STATIC_MAX_N);
+        return static_fail(errbuf, errbuf_len, IA_EINVAL, msg);
+    }
+    if (launch->path != IA_PATH_AUTO)
+        return static_fail(errbuf, errbuf_len, IA_EINVAL, "ia_run_static: launch.path must be IA_PATH_AUTO (it runs the production pair)");
+    ia_ctx cell; /* host-only: parameters and error text; owns no stream, event or device memory */
+    int rc = prepare_cell(&cell, species, trap, De_K, r0_a0, tol);
+    if (rc != IA_OK)
+        return static_fail(errbuf, errbuf_len, rc, "ia_run_static: a species, trap, well-depth, r0 or tolerance value is out of range");
+    IaGen Gn;
+    unsigned long long warn = 0;
+    rc = make_gen(&cell, launch, &Gn, &warn);
+    if (rc != IA_OK) return static_fail(errbuf, errbuf_len, rc, cell.err.c_str());
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || cuda_device < 0 || cuda_device >= ndev || cuda_device >= IA_STATIC_MAX_DEV)
+        return static_fail(errbuf, errbuf_len, IA_EDEVICE, "ia_run_static: no such CUDA device (there is no CPU fallback)");
+    cudaError_t e = cudaSetDevice(cuda_device);
+    if (e != cudaSuccess) return static_fail(errbuf, errbuf_len, IA_ECUDA, cudaGetErrorString(e));
+    const IaStaticDev *D = nullptr;
+    rc = static_device_setup(cuda_device, &D, errbuf, errbuf_len);
+    if (rc != IA_OK) return rc;
+    if (Gn.n == 0) return IA_OK;
+
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    unsigned long long *w = D->scratch->words; /* device addresses: arithmetic only, never dereferenced on the host */
+    IaHand *queue = D->scratch->q;
+    e = cudaMemsetAsync(w, 0, IA_STATIC_WORDS * sizeof(unsigned long long), st);
+    if (e != cudaSuccess) return static_fail(errbuf, errbuf_len, IA_ECUDA, cudaGetErrorString(e));
+    IaOut O;
+    O.records = outputs->records;
+    O.summary = outputs->summary;
+    O.ic_dump = outputs->ic_dump;
+    /* bulk kernel: generates and propagates; a drained warp with at most 16 running lanes -- or any drained warp 4096
+     * iterations on -- hands them to the queue (ia_create's defaults) */
+    IaSched S;
+    std::memset(&S, 0, sizeof(S));
+    S.counter = w + 0;
+    S.n_in = w + 1;
+    S.q_out = queue;
+    S.n_out = w + 2;
+    S.handoff_lanes = 16;
+    S.budget = IA_BULK_BUDGET;
+    S.q_cap = IA_STATIC_MAX_N;
+    S.fault = w + 3;
+    S.n_late = w + 4;
+    S.warn = warn;
+    const unsigned long long full0 = (unsigned long long)D->n_sm * D->kinfo[0].blocks_per_sm;
+    const unsigned long long need0 = (Gn.n + 31ull) / 32ull;
+    e = ia_launch_persistent(1, cell.P, Gn, O, S, (int)(need0 < full0 ? need0 : full0), st);
+    /* cooperative kernel: finishes whatever the queue holds (possibly nothing), one warp per SM sub-partition at most */
+    if (e == cudaSuccess) {
+        IaGen G0;
+        std::memset(&G0, 0, sizeof(G0));
+        IaOut O0 = {nullptr, nullptr, nullptr}; /* every queue entry carries its own output pointers */
+        IaSched C5;
+        std::memset(&C5, 0, sizeof(C5));
+        C5.q_in = queue;
+        C5.n_in = w + 2;
+        C5.counter = w + 5;
+        C5.q_cap = IA_STATIC_MAX_N;
+        C5.fault = w + 3;
+        C5.n_late = w + 4;
+        const unsigned long long sparse = (unsigned long long)D->n_sm * 4ull;
+        const unsigned long long need1 = (Gn.n + 9ull) / 10ull;
+        e = ia_launch_persistent(3, cell.P, G0, O0, C5, (int)(need1 < sparse ? need1 : sparse), st);
+    }
+    if (e != cudaSuccess) {
+        char msg[200];
+        std::snprintf(msg, sizeof(msg), "ia_run_static: kernel launch: %s", cudaGetErrorString(e));
+        return static_fail(errbuf, errbuf_len, IA_ECUDA, msg);
+    }
+    if (!cell.err.empty()) static_fail(errbuf, errbuf_len, IA_OK, cell.err.c_str()); /* the PAPER.md:28 warning */
+    return IA_OK;
+}
