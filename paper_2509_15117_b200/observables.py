@@ -6,12 +6,26 @@ reduction over trajectories that the device has not already done -- array arithm
   maps(...)            the three (theta, phi) images of Fig. 1: chi, log10(number of bounces), min(q, 0.015 a.u.)
   survival_curve(...)  fraction of complexes still alive after t (Fig. 2) from ia_summary.hist_tlife
   power_law_exponent() slope of log S against log t beyond t_min ("after about 20 us ... a power law")
+  heating_scale_uK()   W0^3D of Eq. 3, the energy scale the paper's thresholds are quoted in
 """
 from __future__ import annotations
 
 import numpy as np
 
 Q_CLIP_AU = 0.015   # Fig. 1(d) of the paper clips the momentum transfer at 0.015 a.u. (PAPER.md:24)
+
+
+def heating_scale_uK(m_ion_u: float, m_atom_u: float, alpha_au: float, a_x: float, q_x: float,
+                     omega_rf_au: float) -> float:
+    """Eq. 3 of the paper: W0^3D = 8/(3 pi) (m_a/(m_i+m_a))^(5/3) (m_i^2 w^4 C4 / q_x^2)^(1/3) with the
+    secular frequency w ~ Omega_rf/2 sqrt(a_x + q_x^2/2) and C4 = alpha/2, returned as W0/k_B in
+    microkelvin.  A scale for reading results ("the threshold energy is consistently 2-3 times" W0, PAPER.md:54);
+    nothing in the propagation uses it."""
+    me_per_u, kb_eh_per_k = 1822.888486283, 3.1668115634564e-6   # CODATA 2022
+    m_i, m_a = m_ion_u * me_per_u, m_atom_u * me_per_u
+    w = 0.5 * omega_rf_au * np.sqrt(a_x + 0.5 * q_x * q_x)
+    w0 = 8.0 / (3.0 * np.pi) * (m_a / (m_i + m_a)) ** (5.0 / 3.0) * (m_i * m_i * w ** 4 * (0.5 * alpha_au) / (q_x * q_x)) ** (1.0 / 3.0)
+    return float(w0 / kb_eh_per_k * 1e6)
 
 
 def scattering(records: np.ndarray, ic: np.ndarray, m_atom_me: float):
