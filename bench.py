@@ -12,10 +12,13 @@ trajectories the step before left unfinished, so the power-law tail of trajector
 full warps while new trajectories keep arriving.  The timed region is K consecutive steps of the running stream,
 entered after W warm-up steps (the first of them alone and timed separately: `latency_one_step_alone_ms`) and left
 when the K-th bulk kernel ends; `value` = trajectories FINISHED inside it per second, device-resident.  The
-straggler chain that ends the stream afterwards is timed on its own (`tail`).  `e2e` = the same stream continued
-through ia_submit_host with page-locked HOST buffers (launch descriptor in, 1 GiB of records per step copied
-back inside the timed region).  `roofline` is against the FP64 FMA peak measured live by the library's DFMA
-microbenchmark (MEASURED_PEAKS.json carries no FP64 figure).  Prints ONE JSON line on rank 0.
+straggler chain that ends the stream afterwards is timed on its own (`tail`); `whole_stream` = every trajectory of
+the stream over the time from its first launch to the end of that chain.  `e2e` = a further stream of the same
+shape through ia_submit_host with page-locked HOST buffers (launch descriptor in, 1 GiB of records per step copied
+back), timed from the first submit until ia_wait returns: straggler chain, late records and summaries included
+(`e2e.streaming`: the same leg stopped at ia_sync, i.e. the steady-state rate).  `roofline` is against the FP64 FMA
+peak measured live by the library's DFMA microbenchmark (MEASURED_PEAKS.json carries no FP64 figure), with the
+fraction of the pipe's nominal rate at the measured SM clock beside it.  Prints ONE JSON line on rank 0.
 `--impl reference` times the CPU oracle (test infrastructure; the only other place that may run it).
 """
 from __future__ import annotations
@@ -42,6 +45,13 @@ METRIC = "trajectories/s"
 # count ncu reads off the bulk kernel (sass__inst_executed_per_opcode per warp and step: DFMA 345.0, DMUL 143.6,
 # DADD 33.0; compares are not counted).  Round 1's step needed 886: the error norm and the controller have shed 19.
 FLOP_PER_STEP = 867.0
+# DRAM traffic of the bulk kernel (dram__bytes_read.sum + dram__bytes_write.sum under `ncu --set full`): 125.03 MB for a
+# launch of 2^21 fresh trajectories = 59.6 B per trajectory, against 64 B of record written per trajectory (the kernel
+# reads no input arrays; part of the last records is still in L2 when the kernel ends).  The bench line scales it to its
+# own launch size.  Irrelevant to the bound (FP64 issue).
+TRAFFIC_BYTES_PER_TRAJECTORY = 125030912 / 2097152
+TRAFFIC_SOURCE = ("profiles/r03_k1_raw.csv: 22.24 MB read + 102.79 MB written by one bulk-kernel launch of 2^21 trajectories, "
+                  "scaled per trajectory to this run's launch size")
 ORACLE_SAMPLE_EVERY = 8   # oracle legs on a GRID workload: every 8th grid point in theta and phi (64x64 = 4,096)
 ORACLE_SAMPLE_PHILOX = 8192   # ... on a Philox stream: its first 8,192 indices (reference arm, per step)
 ORACLE_SAMPLE_BASELINE = 32768  # ... and for the one-shot cpu_baseline of our arm
@@ -247,19 +257,24 @@ def run_ours(args):
             dist.barrier(device_ids=[local])
         torch.cuda.synchronize(dev)
 
-    peak = P.ia_fp64_peak(local, 300.0)          # the roofline denominator, measured on this GPU now
+    # the roofline denominator, measured on this GPU now: 2 s of DFMA chains on every SM, SM clock sampled meanwhile
+    peak_clocks = ClockSampler(local)
+    peak_clocks.start()
+    time.sleep(0.3)
+    peak = P.ia_fp64_peak(local, 2000.0)
+    peak_clk = peak_clocks.stop()
     ctx = P.Context(cell.params, device=local)
     if args.handoff >= 0:
         ctx.set_handoff(args.handoff)
-    levels = P.IA_STRAGGLER_LEVELS
+    levels = 1                                   # the library's default (ia_set_chain): one cooperative launch ends the chain
     if args.chain:
         levels, budget = (int(x) for x in args.chain.split(","))
         ctx.set_chain(levels, budget)
     depth = max(0, min(args.pipeline, 64))
-    # the library ends a pipeline by itself after `depth` runs (ia_set_pipeline): keep the end-to-end leg inside it, and
-    # say so if the timed region itself is longer (a straggler chain then falls into it)
+    # the library ends a pipeline by itself after `depth` runs (ia_set_pipeline): keep the end-to-end leg (a stream of
+    # its own) within one, and say so if the timed region itself is longer (a straggler chain then falls into it)
     if depth > 0:
-        Ke = max(0, min(Ke, depth - (W - 1 + K)))
+        Ke = min(Ke, depth)
     chain_in_region = depth > 0 and W - 1 + K > depth
     info = ctx.kernel_info
     # every step of the device leg keeps its own record buffer until the stream is drained (a trajectory in flight
@@ -283,6 +298,8 @@ def run_ours(args):
     alone_t = ctx.timing(0)
     # the stream proper: warm-up steps 1..W-1 fill the pipeline, then the timed region, no join in between
     ctx.set_pipeline(depth)
+    ev_s0, ev_s1 = mk(), mk()
+    ev_s0.record()                                # the stream starts here: W-1 warm-up + K timed steps, then its chain
     for w in range(1, W):
         ctx.run(launch_of(w), records=recs_d[w], summary=summaries[w])
         flush.fill_(w)
@@ -306,8 +323,19 @@ def run_ours(args):
     slots_region = int(mid["slots_bulk"][W:].sum())
     steps_region_all = int(D.all_reduce_sum(steps_region, dev))
 
-    # end to end: the same stream continued through the host entry points, page-locked host buffers: launch
-    # descriptor in, records copied back behind every bulk kernel (inside the timed region)
+    # the end of the device-resident stream: one straggler chain for what the last bulk kernel left
+    t0 = time.perf_counter()
+    ctx.join()
+    ev_s1.record()
+    torch.cuda.synchronize(dev)
+    drain_s = D.all_reduce_max(time.perf_counter() - t0, dev)
+    stream_s = D.all_reduce_max(ev_s0.elapsed_time(ev_s1) * 1e-3, dev)   # first launch of the stream -> end of its chain
+    chain_t = ctx.timing(0)
+    kernel_ms = [ctx.timing(K - 1 - k)["bulk_ms"] for k in range(K)]   # the K timed bulk kernels
+
+    # End to end, a stream of its own through the host entry points with page-locked host buffers: launch descriptor
+    # in, records copied back behind every bulk kernel, and the clock stops when ia_wait returns -- after the straggler
+    # chain, with the late records stored and every summary back on the host.
     e2e = None
     if Ke > 0:
         rec_h = []
@@ -317,36 +345,36 @@ def run_ours(args):
             except RuntimeError:
                 break
         Ke = len(rec_h)
+    if Ke > 0:
+        import ctypes
         sum_h = [torch.zeros(P.SUMMARY_BYTES, dtype=torch.uint8).pin_memory() for _ in range(Ke)]
         cls = [P.make_launch(launch_of(W + K + k)) for k in range(Ke)]
         barrier()
         t0 = time.perf_counter()
         for k in range(Ke):
             P.ia_submit_host(ctx.handle, cls[k], rec_h[k], sum_h[k])
-        ctx.sync()                                                  # every bulk kernel and every copy back has landed
+        ctx.sync()                                                  # every bulk kernel and its copy back has landed
+        sync_s = time.perf_counter() - t0
+        ctx.wait()                                                  # chain, late records, summaries: everything is home
         e2e_s = D.all_reduce_max(time.perf_counter() - t0, dev)
-        import ctypes
-        e2e = None if Ke == 0 else {"value": world * n * Ke / e2e_s, "unit": "trajectories/s", "steps": Ke,
-               "h2d_bytes_per_step": ctypes.sizeof(P.ia_launch),
-               "d2h_bytes_per_step": int(rec_h[0].numel()), "ms_per_step": 1e3 * e2e_s / Ke,
-               "note": "ia_submit_host x steps + ia_sync on the running pipeline: generator mode, so the input of a step is "
-                       "its launch descriptor; records of a step are copied to page-locked host memory behind its bulk "
-                       "kernel; trajectories still in flight then (<= one per lane) report at ia_wait"}
-    # the end of the stream: one straggler chain for what the last bulk kernel left
-    t0 = time.perf_counter()
-    ctx.wait()
-    ctx.join()
-    torch.cuda.synchronize(dev)
-    drain_s = D.all_reduce_max(time.perf_counter() - t0, dev)
-    if Ke > 0:
-        done_h = sum(int(s.numpy().view(P.SUMMARY_DTYPE)[0]["n_done"]) for s in sum_h)
+        sync_s = D.all_reduce_max(sync_s, dev)
+        done_h = sum(int(x.numpy().view(P.SUMMARY_DTYPE)[0]["n_done"]) for x in sum_h)
         assert done_h == Ke * n, (done_h, Ke * n)
-        st = rec_h[-1].numpy().view(P.RECORD_DTYPE)["status"]
-        assert int((st > 4).sum()) == 0
+        for r in rec_h:
+            assert int((r.numpy().view(P.RECORD_DTYPE)["status"] > 4).sum()) == 0
+        e2e_chain = ctx.timing(0)["coop_ms"]
+        e2e = {"value": world * n * Ke / e2e_s, "unit": "trajectories/s", "steps": Ke,
+               "h2d_bytes_per_step": ctypes.sizeof(P.ia_launch),
+               "d2h_bytes_per_step": int(rec_h[0].numel()) + P.SUMMARY_BYTES, "ms_per_step": 1e3 * e2e_s / Ke,
+               "seconds": e2e_s, "chain_ms": e2e_chain,
+               "streaming": {"value": world * n * Ke / sync_s, "seconds": sync_s,
+                             "note": "the same leg stopped at ia_sync: bulk kernels and their copies back done, the "
+                                     "trajectories still in flight (<= one per lane of the grid) and the summaries not yet home"},
+               "note": "a stream of its own: ia_submit_host x steps, then ia_wait; generator mode, so the input of a step is "
+                       "its launch descriptor; records of a step are copied to page-locked host memory behind its bulk kernel; "
+                       "the clock stops when ia_wait returns, i.e. after the straggler chain, the late records and the summaries"}
     fin = view_all()
     assert int(fin["n_done"].sum()) == (W + K) * n, (int(fin["n_done"].sum()), (W + K) * n)
-    chain_t = ctx.timing(0)
-    kernel_ms = [ctx.timing(Ke + K - 1 - k)["bulk_ms"] for k in range(K)]   # the K timed bulk kernels
     bulk_ms = float(np.mean(kernel_ms))
     tot = D.all_reduce_summary(D.sum_summaries(fin[W:]), dev)
     attempted = tot["steps_acc"] + tot["steps_rej"] + tot["steps_loc"]
@@ -363,6 +391,11 @@ def run_ours(args):
     value = finished / region_s
     achieved_tflops = FLOP_PER_STEP * steps_region / (sum(kernel_ms) * 1e-3) / 1e12
     whole_tflops = FLOP_PER_STEP * steps_region / region_s / 1e12
+    # the FP64 pipe's own rate: 64 FMA per SM and clock (B200_PROFILING / B300_MICROARCH unit counts) at the SM clock
+    # nvidia-smi reported during the timed region; the DFMA microbenchmark reaches about 92 % of it
+    sm_mhz = clk.get("sm_mhz") or clk.get("sm_max_mhz") or peak_clk.get("sm_mhz") or 1965.0
+    nominal_tflops = info["bulk"]["n_sm"] * 64 * 2 * sm_mhz * 1e6 / 1e12
+    n_stream = (W - 1 + K) * n
     line = {
         "metric": METRIC, "value": value, "unit": "trajectories/s", "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": 1e3 * region_s / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -371,7 +404,7 @@ def run_ours(args):
                    "trajectories_per_step_per_gpu": n, "parallelism": f"dp{world}",
                    "timed_region": "K consecutive steps of a running pipeline (ia_set_pipeline): entered after W warm-up steps "
                                    "without a join, left when the K-th bulk kernel ends; value = trajectories finished inside it; "
-                                   "the straggler chain that ends the stream is timed separately (tail)",
+                                   "the straggler chain that ends the stream is timed separately (tail) and counted in whole_stream",
                    "l2": "flushed between timed iterations (256 MiB write); the kernel reads no input arrays",
                    "pipeline_depth": depth, "chain_inside_timed_region": bool(chain_in_region),
                    "rtol": cell.params.rtol, "atol": cell.params.atol, "t_max_rf": cell.params.t_max_rf},
@@ -382,27 +415,43 @@ def run_ours(args):
         "one_step_alone": {"bulk_ms": alone_t["bulk_ms"], "chain_ms": alone_t["coop_ms"],
                            "trajectories_per_s": n / (alone_ms * 1e-3)},
         "p_complex": tot["n_complex"] / max(tot["n_done"], 1), "n_status": tot["n_status"],
-        "roofline": {"bound": "alu", "achieved": achieved_tflops, "peak": peak["tflops"], "unit": "TFLOP/s",
-                     "frac": achieved_tflops / peak["tflops"],
-                     "traffic": None,
-                     "peak_source": "ia_fp64_peak (DFMA chains on all SMs, measured in this run); nominal 37.2",
+        "roofline": {"bound": "alu", "achieved": achieved_tflops, "peak": nominal_tflops, "unit": "TFLOP/s",
+                     "frac": achieved_tflops / nominal_tflops,
+                     "peak_source": "FP64 pipe at its nominal rate: SMs x 64 FMA/clk x 2 x the median SM clock nvidia-smi "
+                                    "reported in the timed region (unit counts: /opt/skills/guides; DESIGN.md 'Roofline'); ncu "
+                                    "counts the pipe against the same rate (profiles/r03_ncu.md)",
+                     "peak_measured_dfma": peak["tflops"], "frac_of_measured_dfma": achieved_tflops / peak["tflops"],
+                     "peak_measured_dfma_source": "ia_fp64_peak: 2 s of independent DFMA chains on every SM in this run; it "
+                                                  "keeps the pipe 92.2 % busy (ncu, profiles/r03_k4_raw.csv)",
+                     "peak_elapsed_ms": peak["elapsed_ms"], "peak_clocks": peak_clk,
+                     "traffic": TRAFFIC_BYTES_PER_TRAJECTORY * n, "traffic_source": TRAFFIC_SOURCE,
+                     "progress_metric": "rk_steps_per_s (flops are executed flops: frac rises if a step does more arithmetic)",
                      "flop_per_attempted_step": FLOP_PER_STEP, "kernel": "ia_persistent_kernel<1, IA_SRC_BOTH> (bulk)",
                      "kernel_ms": bulk_ms, "steps_in_kernel": steps_region / K,
                      "share_of_step_time": sum(kernel_ms) * 1e-3 / region_s,
                      # share of the kernel's lane-steps (32 per warp and attempt) that advanced a trajectory
                      "lane_efficiency": steps_region / max(slots_region, 1)},
         # every attempted step executed inside the timed region over the whole region
-        "whole_step": {"achieved": whole_tflops, "peak": peak["tflops"], "unit": "TFLOP/s",
-                       "frac": whole_tflops / peak["tflops"], "rk_steps": steps_region, "seconds": region_s},
+        "whole_step": {"achieved": whole_tflops, "peak": nominal_tflops, "unit": "TFLOP/s",
+                       "frac": whole_tflops / nominal_tflops,
+                       "frac_of_measured_dfma": whole_tflops / peak["tflops"],
+                       "rk_steps": steps_region, "seconds": region_s},
+        # the whole device-resident stream, chain included: every trajectory of the W-1 warm-up and K timed steps over the
+        # time from the first launch of the stream to the end of its straggler chain
+        "whole_stream": {"value": world * n_stream / stream_s, "unit": "trajectories/s", "trajectories_per_gpu": n_stream,
+                         "seconds": stream_s, "steps": W - 1 + K},
         # the end of the stream: a trajectory is a serial chain, so the chain lasts as long as the longest one left
-        "tail": {"kernel": f"ia_persistent_kernel<3, IA_SRC_QUEUE> (cooperative, 3 lanes per trajectory), chain of {levels} launches",
+        "tail": {"kernel": f"chain of {2 + levels} launches: ia_persistent_kernel<1, IA_SRC_BOTH> over a full grid (stage A), the "
+                           f"same with one warp per SM sub-partition (stage B), ia_persistent_kernel<3, IA_SRC_QUEUE> "
+                           f"(cooperative, 3 lanes per trajectory, one warp per sub-partition) x {levels} (stage C)",
+                 "launches": 2 + levels,
                  "chain_ms": chain_t["coop_ms"], "drain_wall_ms": 1e3 * drain_s,
                  "share_of_step_time": 0.0,
                  "share_of_stream_time": chain_t["coop_ms"] * 1e-3 / (region_s + chain_t["coop_ms"] * 1e-3),
                  "longest_trajectory_steps_last_step": longest,
                  "note": "outside the timed region; paid once per stream, whatever its length (DESIGN.md 'Tail')"},
         "attempted_steps_of_timed_batches": attempted,
-        "kernel_info": info, "clocks": clk, "e2e": e2e, "gpu_launches": K,
+        "kernel_info": info, "clocks": clk, "e2e": e2e, "gpu_launches": K,   # the K bulk kernels of the timed region (the chain and the e2e leg are outside it)
     }
     if not args.no_cpu_baseline and world == 1:
         s = oracle_sample(cell, args.n_side, ORACLE_SAMPLE_BASELINE)

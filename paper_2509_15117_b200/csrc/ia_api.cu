@@ -31,7 +31,7 @@ struct IaKernelInfo {
 #define IA_NSTAGE 3         /* device staging buffers of the host entry points */
 
 /* The straggler chain.  What decides the latency of a step is how many warps share an SM
- * sub-partition (measured, profiles/r02_latency_vs_occupancy.md: bulk layout 2.61 / 1.84 / 1.14 us per step at
+ * sub-partition (measured, profiles/r02_summary.md section 4: bulk layout 2.61 / 1.84 / 1.14 us per step at
  * 3 / 2 / 1 warps, cooperative layout 1.01 us at 1 warp with a third of the trajectories per warp).  The chain
  * therefore moves what is left into ever fewer warps, by COUNT: stage A = the bulk kernel over a full grid until
  * at most 32 x 4 x #SM trajectories run; stage B = the bulk kernel with one warp per sub-partition until at most

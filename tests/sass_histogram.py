@@ -1,12 +1,12 @@
 """Opcode histogram of the step loop of a persistent kernel, from `cuobjdump -sass` of the built library.
 
-    python -m paper_2509_15117_b200.sass_histogram [bulk|coop]
+    python tests/sass_histogram.py [bulk|coop]
 
 The step loop is the innermost loop that contains the Runge-Kutta attempt: the backward branch with the smallest
 span among those that enclose at least six MUFU.RCP64H (one reciprocal per stage).  Prints the FP64-pipe count
 (DFMA + DMUL + DADD + DSETP), the other opcodes and the local-memory instructions (LDL / STL: spills, must be 0).
-The count is static: rarely taken branches inside the loop are included.  Reporting only: nothing here is used by the
-library.
+The count is static: rarely taken branches inside the loop are included.  Test infrastructure (tests/test_host_logic.py) and reporting
+only: nothing here is used by the library.
 """
 from __future__ import annotations
 
@@ -16,7 +16,7 @@ import subprocess
 import sys
 from pathlib import Path
 
-LIB = Path(__file__).resolve().parent / "libia_b200.so"
+LIB = Path(__file__).resolve().parent.parent / "paper_2509_15117_b200" / "libia_b200.so"
 KERNELS = {"bulk": "ia_persistent_kernelILi1ELi2", "coop": "ia_persistent_kernelILi3ELi1"}
 
 
@@ -65,7 +65,7 @@ def main():
     print(f"  flops per attempted step counted from SASS: {2 * hist['DFMA'] + hist['DMUL'] + hist['DADD']}")
     print(f"  STATIC count: the loop body holds both branches of the error norm (the general tree is not taken in these "
           f"units) and the rarely taken event / termination branch; the instructions a step executes are counted by "
-          f"ncu (profiles/r02b_k1_ncu.md)")
+          f"ncu (profiles/r02_summary.md section 3, profiles/r03_ncu.md)")
     print(f"  issue slots if every instruction of the body ran: 2 x {fp64} + {len(body) - fp64} = "
           f"{2 * fp64 + len(body) - fp64}")
 

@@ -271,7 +271,7 @@ def test_persistent_kernels_use_no_local_memory():
     if shutil.which("cuobjdump") is None:
         pytest.skip("cuobjdump not on PATH")
     import paper_2509_15117_b200 as P
-    from paper_2509_15117_b200 import sass_histogram as H
+    import sass_histogram as H          # tests/sass_histogram.py
     P.load()
     for kernel, fp64_min in (("bulk", 550), ("coop", 280)):
         ins = H.instructions(kernel)
