@@ -134,7 +134,8 @@ typedef struct {
     uint32_t steps_acc; /* accepted RK steps                                                        */
     uint16_t steps_rej; /* rejected RK steps, saturating at 65535                                   */
     uint8_t status;     /* 0 escaped (|d| > r0 after closest approach), 1 t_max reached,
-                           2 step size underflow, 3 non-finite initial state, 4 max_steps          */
+                           2 step size underflow, 3 non-finite initial state (or exit-localisation
+                           step), 4 max_steps                                                      */
     uint8_t n_loc;      /* exit-localisation iterations used (R7)                                   */
 } ia_record;
 

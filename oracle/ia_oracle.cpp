@@ -279,6 +279,12 @@ int run_one(const Derived &D, const double y0[12], double phase, oracle_outcome 
                 }
                 out->n_loc = nloc;
                 out->steps_rej = (uint32_t)(attempts - out->steps_acc);
+                if (!all_finite(ynew)) {
+                    /* R7: a localisation step that is not finite (it only shortens a finite accepted step, so this is
+                     * not reachable from finite states) is not an escape: status 3 at the last state inside */
+                    finish(D, out, 3, y, now(), t_first, t_last);
+                    return 0;
+                }
                 const double t_exit = now() + hk;
                 record(t_exit, ynew);
                 finish(D, out, 0, ynew, t_exit, t_first, t_last);

@@ -125,6 +125,9 @@ IA_DEV double ia_inv_fifth_root(double x) {
     const float xf = (float)x;
     float lf;
     asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(lf) : "f"(xf));
+    /* 0 <= x < 2^-126 flushes to lg2 = -inf, which would come out as -inf below (0 itself as NaN): keep the seed finite,
+     * the result is then huge and the step law's cap of 5 applies.  No effect on any x a float can hold. */
+    lf = fmaxf(lf, -126.0f);
     float sf;
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(sf) : "f"(-0.2f * lf));
     const double y = (double)sf;

@@ -569,9 +569,12 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
         const double hs = h; /* the step just attempted */
         const double denr = P.rtol * so.err.den;
         const bool accept = so.finite && (so.err.num <= denr);
-        /* 0.8 (rtol/err)^(1/5).  err = 0 gives NaN and err = NaN or inf gives NaN or 0: ia_min / ia_max below return
-         * their second operand then, i.e. growth by 5 and shrinkage by 10 as the step law says */
-        const double fac = 0.8 * ia_inv_fifth_root(so.err.num * ia_rcp(denr));
+        /* 0.8 (rtol/err)^(1/5).  err = 0 (or below 2^-126 rtol) gives a huge factor and err = NaN or inf gives NaN or 0:
+         * ia_min / ia_max below cap the former at 5 and return their second operand for NaN, i.e. growth by 5 and
+         * shrinkage by 10 as the step law says.  A step that is not finite shrinks by 10 whatever its error norm reads
+         * (a NaN in a component the norm's maxima drop must not let the step grow). */
+        const double fac0 = 0.8 * ia_inv_fifth_root(so.err.num * ia_rcp(denr));
+        const double fac = so.finite ? fac0 : 0.1;
         const bool acc = run && accept, rej = run && !accept;
         steps_acc += acc ? 1u : 0u;
         const bool neg_new = so.s_new < 0.0;
@@ -625,12 +628,14 @@ ia_persistent_kernel(const __grid_constant__ IaParams P, const __grid_constant__
                     sh.loc_hi[threadIdx.x] = hi;
                     mode = MODE_LOC;
                 } else {
-                    fin = 0;
-                    t_fin = now + hs;
+                    /* a localisation step that is not finite (unreachable from a finite accepted step, since it only
+                     * shortens it) must not leave as an escape with a non-finite energy: status 3 at the last state */
+                    fin = so.finite ? 0 : 3;
+                    t_fin = so.finite ? now + hs : now;
                 }
             }
-            if (fin == 0) {
-                /* ended at the localised exit */
+            if (fin == 0 || fin == 3) {
+                /* ended at the localised exit (or with a localisation step that is not finite) */
             } else if (commit && last) {
                 fin = 1;
                 t_fin = P.t_max;

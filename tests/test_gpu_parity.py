@@ -959,3 +959,102 @@ def test_no_out_of_bounds_writes_guard_zones(P):
         _, s, _ = ctx.run_sync(th.launch)
         assert int(s["n_done"]) == 1000
         ctx.debug_check()
+
+
+# ---------------------------------------------------------------------------------------------
+# the error norm's general branch, and the step law at its edges
+# ---------------------------------------------------------------------------------------------
+def test_error_norm_general_branch_against_the_oracle(P):
+    """Every other GPU test keeps atol/rtol = 1e-2 a.u. far above the velocities (~1e-7 a.u.), so the error norm takes
+    its warp-uniform fast path (velocity scale = thr).  With atol = 1e-22 the threshold is 1e-12: every velocity scale
+    is max(|v|, |v_new|), i.e. the general comparison tree, in the one-step map (all three arithmetic variants: new
+    state to 1e-12, err to 1e-5 of itself, R5/R12) and in adaptive runs of config 0 (identical step counts, final
+    observables at the bars of test_config0_adaptive_parity_full)."""
+    cell = I.config0()
+    cell = replace(cell, params=replace(cell.params, atol=1e-22))
+    tf, ph, y, h = _sampled_states(cell, n_traj=4)
+    assert np.abs(y[:, 9:12]).max(axis=1).min() > 100 * cell.params.atol / cell.params.rtol      # thr is below every |v_a|
+    ref = np.empty_like(y); eref = np.empty(len(y))
+    for k in range(len(y)):
+        yn, e = O.step(cell.params, tf[k], ph[k], y[k], h[k])
+        ref[k] = yn
+        eref[k] = O.err_norm(cell.params, y[k], yn, e)
+    with P.Context(cell.params) as ctx:
+        for variant in (0, 1, 2):
+            got, err = ctx.step_map(tf, ph, y, h, variant=variant)
+            rel = block_rel(got, ref, 1e-3 * np.linalg.norm(y[:, 9:12], axis=1).max())
+            assert rel.max() <= 1e-12, (variant, rel.max(axis=0))
+            # err to 1e-5 of itself as in test_one_step_map_1e12, plus the absolute floor of a sum with cancelling
+            # weights where the step is tiny (the first steps: err ~ 1e-11, difference 2e-16)
+            assert np.all(np.abs(err - eref) <= 1e-5 * eref + 1e-15), (variant, np.max(np.abs(err - eref) / eref))
+        n = 256
+        launch = replace(cell.launch, n=n)
+        runs = {path: ctx.run_sync(replace(launch, path=path))[0] for path in (0, 1, 2)}
+    _assert_records_identical(runs[0], runs[1])
+    _assert_records_identical(runs[0], runs[2])
+    rec = runs[0]
+    o = O.run_generated(cell.params, launch, nthreads=NTHREADS)
+    assert np.array_equal(rec["status"], o["status"].astype(np.uint8)) and np.array_equal(rec["n_coll"], o["n_coll"])
+    same = (rec["steps_acc"] == o["steps_acc"]) & (rec["steps_rej"] == o["steps_rej"])
+    assert same.sum() >= n - 2, int(same.sum())
+    e_t = np.max(np.abs(rec["t_dwell"][same] - o["t_dwell"][same]) / o["t_dwell"][same])
+    e_k = np.max(np.abs(rec["ke_ion"][same] - o["ke_ion"][same]) / o["ke_ion"][same])
+    print(f"\ngeneral norm branch (atol 1e-22): {int(same.sum())}/{n} identical step sequences, t_dwell {e_t:.2e} ke_ion {e_k:.2e}; "
+          f"accepted steps {int(rec['steps_acc'].mean())} (1e-12: {int(O.run_generated(I.config0().params, replace(launch, n=8))['steps_acc'].mean())})")
+    assert e_t < 1e-8 and e_k < 1e-7
+
+
+def test_a_fast_warp_mate_does_not_change_its_neighbours(P):
+    """Which branch of the error norm a trajectory takes depends on its warp-mates (the fast path needs every lane of
+    the warp below thr).  32 explicit initial conditions with thr = 1e-7 a.u. between two populations: 31 slow atoms
+    (Li at 1 uK, |v| = 2.2e-8: below thr until the C4 attraction has sped them up, at r ~ 1000 a0) and, in the second
+    run, one fast atom (100 uK, |v| = 2.2e-7) in lane 7, which forces the general tree on the whole warp from the first step.  The 31 others must come out
+    bit-identical -- the two branches pick the maximum of the same twelve ratios."""
+    base = I.config0()
+    p = replace(base.params, atol=1e-17, t_max_rf=200.0)        # thr = atol/rtol = 1e-7
+    slow = replace(base.launch, n=32, n_theta=4, n_phi=8, E_min_uK=1.0, E_max_uK=1.0)
+    y_slow, ph, _ = O.generate(p, slow, np.arange(32))
+    y_fast, _, _ = O.generate(p, replace(slow, E_min_uK=100.0, E_max_uK=100.0), np.arange(32))
+    thr = p.atol / p.rtol
+    assert np.abs(y_slow[:, 9:12]).max() < thr < np.abs(y_fast[7, 9:12]).max()
+    mixed = y_slow.copy()
+    mixed[7] = y_fast[7]
+    with P.Context(p) as ctx:
+        L = I.Launch(mode=I.MODE_EXPLICIT, n=32, path=1)         # one warp of the bulk kernel to the end
+        a, _, _ = ctx.run_sync(L, y0=y_slow, phase=ph)
+        b, _, _ = ctx.run_sync(L, y0=mixed, phase=ph)
+    others = np.ones(32, dtype=bool)
+    others[7] = False
+    assert a["steps_acc"][others].min() > 50 and not np.array_equal(a[7:8].tobytes(), b[7:8].tobytes())
+    _assert_records_identical(a[others], b[others])
+    # and the slow ones agree with the oracle (whose norm is the plain twelve-way maximum)
+    o = O.run_explicit(p, y_slow, ph, nthreads=NTHREADS)
+    assert np.array_equal(a["status"], o["status"].astype(np.uint8))
+    same = (a["steps_acc"] == o["steps_acc"]) & (a["steps_rej"] == o["steps_rej"])
+    assert same.sum() >= 30
+    # E is ten times below config 0's, and round-off is amplified in proportion to D_e/E (R15): ten times config 0's bar
+    assert np.max(np.abs(a["t_dwell"][same] - o["t_dwell"][same]) / o["t_dwell"][same]) < 1e-7
+
+
+def test_step_law_when_the_error_underflows(P):
+    """An error norm that is positive but below what a float can hold (the first operand of the fifth root's FP32 seed)
+    is a step of no measurable error: the step grows by 5 up to h_max, as for err = 0 (ode45 [23], R5).  A polarisability
+    of 1e-60 a.u. (no interaction to speak of), the atom 4000 a0 out with a velocity of 1e-45 a.u., the ion at rest at the
+    trap centre: the error estimate is of order 1e-57 of the scale (oracle: err = 4.9e-57, 24 steps of T_rf/4 to t_max).
+    Before round 3 the seed was infinite there, the next step size NaN and the record a spurious status 2.  Both sides
+    must reach t_max with the same steps."""
+    base = I.config1(8)
+    p = replace(base.params, t_max_rf=6.0, alpha_au=1e-60)
+    y = np.zeros((3, 12))
+    for k in range(3):
+        y[k, 3 + k] = 4000.0                # atom on axis k, 4000 a0 out
+        y[k, 9 + k] = -1e-45                # drifting in at 1e-45 a.u.
+    ph = np.array([0.0, 1.0, 2.0])
+    with P.Context(p) as ctx:
+        rec, summ, _ = ctx.run_sync(I.Launch(mode=I.MODE_EXPLICIT, n=3), y0=y, phase=ph)
+    o = O.run_explicit(p, y, ph, nthreads=1)
+    print(f"\nunderflowing error: status {rec['status']} steps {rec['steps_acc']} rejected {rec['steps_rej']}; oracle "
+          f"status {o['status']} steps {o['steps_acc']}")
+    assert np.all(o["status"] == 1) and np.all(rec["status"] == 1)
+    assert np.array_equal(rec["steps_acc"], o["steps_acc"]) and np.all(rec["steps_rej"] == 0)
+    assert np.array_equal(rec["t_dwell"], o["t_dwell"])
