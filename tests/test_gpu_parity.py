@@ -577,26 +577,28 @@ def test_every_cell_of_configs_2_and_3_against_the_oracle(P, which):
     (config 3's D_e = 10 K and 100 K rows with t_max cut to 300 and 100 T_rf on both sides so that the oracle
     finishes: a complex still bound then counts as one).  Per cell: statuses and bounce counts of the single-bounce
     trajectories identical, their dwell times at the round-off floor of the cell, the number of complexes inside
-    the 99.9 % two-proportion interval (45 cells: one re-draw with a new seed allowed per cell, R15), and the
-    trend the paper states across cells checked on the GPU numbers."""
+    the two-proportion interval at a family-wise 99 % over the cells of the config (Bonferroni: no re-draws), the
+    standardised differences of all cells pooled into one chi-square at 99 %, every cell beyond its own 99 %
+    printed, and the trend the paper states across cells checked on the GPU numbers."""
+    from scipy import stats
     n = 1024
     cells = I.config2(n_per_cell=n) if which == "config2" else I.config3(n_per_cell=n)
     if which == "config3":
         cut = {10.0: 300.0, 100.0: 100.0}
         cells = [replace(c, params=replace(c.params, t_max_rf=cut.get(c.params.De_K, c.params.t_max_rf))) for c in cells]
-    z999 = 3.2905267314919255
-    p_gpu = {}
+    z_fw = float(stats.norm.ppf(1.0 - 0.01 / (2 * len(cells))))     # 3.69 for 25 cells, 3.66 for 20
+    p_gpu, z_cells = {}, []
     for cell in cells:
         launch = cell.launch
-        for attempt in range(2):
-            with P.Context(cell.params) as ctx:
-                rec, summ, _ = ctx.run_sync(launch)
-            ref = O.run_generated(cell.params, launch, nthreads=NTHREADS)
-            k_g, k_o = int((rec["n_coll"] >= 2).sum()), int((ref["n_coll"] >= 2).sum())
-            ok, d, half = S.two_proportion_ok(k_g, n, k_o, n, z999)
-            if ok:
-                break
-            launch = replace(launch, seed=launch.seed + 1)
+        with P.Context(cell.params) as ctx:
+            rec, summ, _ = ctx.run_sync(launch)
+        ref = O.run_generated(cell.params, launch, nthreads=NTHREADS)
+        k_g, k_o = int((rec["n_coll"] >= 2).sum()), int((ref["n_coll"] >= 2).sum())
+        ok, d, half = S.two_proportion_ok(k_g, n, k_o, n, z_fw)
+        if k_g + k_o > 0:
+            z_cells.append(d / (half / z_fw))
+            if abs(z_cells[-1]) > S.Z99:
+                print(f"\n{cell.name}: complexes GPU {k_g} oracle {k_o} of {n}: z = {z_cells[-1]:+.2f} (beyond the cell's own 99 %)")
         assert ok, (cell.name, k_g, k_o, half)
         assert int(summ["n_done"]) == n and int(summ["n_complex"]) == k_g
         reg = (ref["n_coll"] <= 1) & (rec["n_coll"] <= 1)
@@ -608,7 +610,12 @@ def test_every_cell_of_configs_2_and_3_against_the_oracle(P, which):
         floor = 1e-8 if cell.params.De_K <= 1.0 else (1e-7 if cell.params.De_K <= 10.0 else 1e-5)
         assert same.sum() >= 0.9 * esc.sum() and np.median(e_t) <= floor, (cell.name, same.sum(), esc.sum(), np.median(e_t))
         p_gpu[cell.name] = k_g / n
-    print(f"\n{which}: P(complex) on the first {n} indices of every cell: " + ", ".join(f"{k.split('_', 1)[1]} {v:.3f}" for k, v in p_gpu.items()))
+    # all cells together: the standardised differences are at most unit normal (the two sides share their initial
+    # conditions, so they are less spread than independent samples would be): chi-square at 99 %
+    chi2 = float(np.sum(np.square(z_cells)))
+    assert chi2 <= stats.chi2.ppf(0.99, max(len(z_cells), 1)), (chi2, len(z_cells))
+    print(f"\n{which}: chi-square of the standardised P(complex) differences over {len(z_cells)} cells with complexes: {chi2:.1f}")
+    print(f"{which}: P(complex) on the first {n} indices of every cell: " + ", ".join(f"{k.split('_', 1)[1]} {v:.3f}" for k, v in p_gpu.items()))
     if which == "config2":
         assert all(p_gpu[f"config2_Li7_{E:g}uK"] == 0.0 for E in I.ENERGIES_UK)            # no complexes for Li head-on
         assert p_gpu["config2_Na23_1uK"] < p_gpu["config2_K39_1uK"] < p_gpu["config2_Cs133_1uK"] + 0.05   # heavier: more
