@@ -289,7 +289,9 @@ int ia_get_last_timing(ia_ctx *ctx, double *bulk_ms, double *coop_ms);
  * tflops = 2 * DFMA/s / 1e12; elapsed_ms = CUDA-event time of the timed launch. */
 int ia_fp64_peak(int cuda_device, double target_ms, double *tflops, double *elapsed_ms);
 
-/* Latency microbenchmark (the floor of the straggler chain): one warp, one dependent chain.
+/* Latency microbenchmark behind the numbers DESIGN.md "Tail" argues from (measured on B200: 8 cycles per dependent DFMA,
+ * 39 per reciprocal + DADD; profiles/r02_summary.md section 4 -- the lone warp of the straggler chain is bound by its
+ * in-order instruction stream, not by the step's arithmetic chain): one warp, one dependent chain.
  * cycles_dfma = SM cycles per dependent DFMA; cycles_rcp_add = SM cycles per reciprocal as the right-hand side
  * computes it (MUFU.RCP64H and three dependent DFMA) followed by one dependent DADD.  Host pointers. */
 int ia_fp64_latency(int cuda_device, double *cycles_dfma, double *cycles_rcp_add);

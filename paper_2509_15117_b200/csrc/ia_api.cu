@@ -158,26 +158,11 @@ static int fail_inval(ia_ctx *c, const char *what) {
     return IA_EINVAL;
 }
 
-extern "C" {
-
-const char *ia_strerror(int code) {
-    switch (code) {
-    case IA_OK: return "ok";
-    case IA_EINVAL: return "invalid argument";
-    case IA_ENOMEM: return "out of memory";
-    case IA_ECUDA: return "CUDA runtime error";
-    case IA_EDEVICE: return "no compute-capability-10.x CUDA device (there is no CPU fallback)";
-    default: return "unknown error code";
-    }
-}
-
-const char *ia_last_error(const ia_ctx *ctx) { return ctx ? ctx->err.c_str() : ""; }
-
-int ia_create(ia_ctx **out, const ia_species *sp, const ia_trap *tr, double De_K, double r0_a0, const ia_tol *tol,
-              int cuda_device) {
-    if (!out) return IA_EINVAL;
-    *out = nullptr;
-    if (!sp || !tr) return IA_EINVAL;
+/* a1: parameter preparation (BASELINE.json north_star) -- range checks, defaults of the tolerances and
+ * the derived constants of one cell (host arithmetic only: no CUDA call).  *w_harm = |q_x| Omega / 2^(3/2), the ion's trap
+ * frequency in thermal runs.  Shared by ia_create and ia_run_static. */
+static int prepare_cell(IaParams *Pout, double derived[16], double *w_harm, const ia_species *sp, const ia_trap *tr,
+                        double De_K, double r0_a0, const ia_tol *tol) {
     ia_tol T;
     std::memset(&T, 0, sizeof(T));
     if (tol) T = *tol;
@@ -196,19 +181,7 @@ int ia_create(ia_ctx **out, const ia_species *sp, const ia_trap *tr, double De_K
     if (!(T.rtol >= 1e-13 && T.rtol <= 1e-3) || !pos(T.atol) || !pos(T.t_max_rf) ||
         !(T.h_max_rf > 0.0 && T.h_max_rf <= 0.25) || !pos(T.r_coll_a0) || T.max_steps > (1ull << 32) - 1)
         return IA_EINVAL;
-
-    int ndev = 0;
-    if (cudaGetDeviceCount(&ndev) != cudaSuccess || cuda_device < 0 || cuda_device >= ndev) return IA_EDEVICE;
-    cudaDeviceProp prop;
-    if (cudaGetDeviceProperties(&prop, cuda_device) != cudaSuccess) return IA_EDEVICE;
-    if (prop.major != 10) return IA_EDEVICE; /* sm_100a only: no fallback path */
-
-    ia_ctx *c = new (std::nothrow) ia_ctx;
-    if (!c) return IA_ENOMEM;
-    c->device = cuda_device;
-
-    /* a1: parameter preparation (BASELINE.json north_star) */
-    IaParams &P = c->P;
+    IaParams &P = *Pout;
     std::memset(&P, 0, sizeof(P));
     P.m_i = sp->m_ion_u * ME_PER_U;
     P.m_a = sp->m_atom_u * ME_PER_U;
@@ -230,7 +203,7 @@ int ia_create(ia_ctx **out, const ia_species *sp, const ia_trap *tr, double De_K
         P.ka[k] = -tr->a[k] * (P.omega * P.omega / 4.0);
         P.kq[k] = -2.0 * tr->q[k] * (P.omega * P.omega / 4.0);
     }
-    c->w_harm = std::fabs(tr->q[0]) * P.omega / std::pow(2.0, 1.5);
+    *w_harm = std::fabs(tr->q[0]) * P.omega / std::pow(2.0, 1.5);
     P.rtol = T.rtol;
     P.atol = T.atol;
     P.thr = T.atol / T.rtol;
@@ -248,8 +221,47 @@ int ia_create(ia_ctx **out, const ia_species *sp, const ia_trap *tr, double De_K
     P.n_near = T.t_max_rf > 2.0 ? (unsigned)std::floor(std::fmin(T.t_max_rf - 2.0, 4294967295.0)) : 0u;
     const double d[16] = {P.m_i, P.m_a, P.C4, P.C8, P.De, P.r_e, P.omega, P.T_rf,
                           P.thr, P.h_max, P.h_min, P.t_max, P.r0, P.r_coll, P.rtol, P.atol};
-    std::memcpy(c->derived, d, sizeof(d));
+    std::memcpy(derived, d, sizeof(d));
+    return IA_OK;
+}
 
+
+extern "C" {
+
+const char *ia_strerror(int code) {
+    switch (code) {
+    case IA_OK: return "ok";
+    case IA_EINVAL: return "invalid argument";
+    case IA_ENOMEM: return "out of memory";
+    case IA_ECUDA: return "CUDA runtime error";
+    case IA_EDEVICE: return "no compute-capability-10.x CUDA device (there is no CPU fallback)";
+    default: return "unknown error code";
+    }
+}
+
+const char *ia_last_error(const ia_ctx *ctx) { return ctx ? ctx->err.c_str() : ""; }
+
+int ia_create(ia_ctx **out, const ia_species *sp, const ia_trap *tr, double De_K, double r0_a0, const ia_tol *tol,
+              int cuda_device) {
+    if (!out) return IA_EINVAL;
+    *out = nullptr;
+    if (!sp || !tr) return IA_EINVAL;
+    /* a1, and with it the argument checks: they answer before any device is looked at */
+    IaParams P0;
+    double derived[16], w_harm = 0.0;
+    if (prepare_cell(&P0, derived, &w_harm, sp, tr, De_K, r0_a0, tol) != IA_OK) return IA_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || cuda_device < 0 || cuda_device >= ndev) return IA_EDEVICE;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, cuda_device) != cudaSuccess) return IA_EDEVICE;
+    if (prop.major != 10) return IA_EDEVICE; /* sm_100a only: no fallback path */
+
+    ia_ctx *c = new (std::nothrow) ia_ctx;
+    if (!c) return IA_ENOMEM;
+    c->device = cuda_device;
+    c->P = P0;
+    c->w_harm = w_harm;
+    std::memcpy(c->derived, derived, sizeof(derived));
     c->n_sm = prop.multiProcessorCount;
     cudaError_t e = cudaSetDevice(cuda_device);
     if (e == cudaSuccess) e = guarded_malloc(c, (void **)&c->counters, IA_COUNTER_RING * 4 * sizeof(unsigned long long));
@@ -976,71 +988,6 @@ static int static_device_setup(int dev, const IaStaticDev **out, char *errbuf, s
     return IA_OK;
 }
 
-/* a1 for a caller without a ctx: the checks and the derived constants of ia_create (BASELINE.json
- * north_star), written into a host-only ia_ctx that owns no CUDA resource */
-static int prepare_cell(ia_ctx *c, const ia_species *sp, const ia_trap *tr, double De_K, double r0_a0, const ia_tol *tol) {
-    ia_tol T;
-    std::memset(&T, 0, sizeof(T));
-    if (tol) T = *tol;
-    if (T.rtol == 0.0) T.rtol = 1e-10;
-    if (T.atol == 0.0) T.atol = 1e-12;
-    if (T.t_max_rf == 0.0) T.t_max_rf = 1e4;
-    if (T.h_max_rf == 0.0) T.h_max_rf = 0.25;
-    if (T.r_coll_a0 == 0.0) T.r_coll_a0 = 500.0;
-    if (T.max_steps == 0) T.max_steps = 1ull << 31;
-    auto pos = [](double v) { return std::isfinite(v) && v > 0.0; };
-    if (!pos(sp->m_ion_u) || !pos(sp->m_atom_u) || !pos(sp->alpha_au) || !pos(De_K) || !pos(r0_a0) ||
-        !pos(tr->omega_rf_au))
-        return IA_EINVAL;
-    for (int k = 0; k < 3; ++k)
-        if (!std::isfinite(tr->a[k]) || !std::isfinite(tr->q[k])) return IA_EINVAL;
-    if (!(T.rtol >= 1e-13 && T.rtol <= 1e-3) || !pos(T.atol) || !pos(T.t_max_rf) ||
-        !(T.h_max_rf > 0.0 && T.h_max_rf <= 0.25) || !pos(T.r_coll_a0) || T.max_steps > (1ull << 32) - 1)
-        return IA_EINVAL;
-    IaParams &P = c->P;
-    std::memset(&P, 0, sizeof(P));
-    P.m_i = sp->m_ion_u * ME_PER_U;
-    P.m_a = sp->m_atom_u * ME_PER_U;
-    P.inv_m_a = 1.0 / P.m_a;
-    P.neg_inv_m_i = -1.0 / P.m_i;
-    P.C4 = sp->alpha_au / 2.0;
-    P.De = De_K * KB_EH_PER_K;
-    P.C8 = P.C4 * P.C4 / (4.0 * P.De);
-    P.r_e = std::pow(2.0 * P.C8 / P.C4, 0.25);
-    P.c8x8 = 8.0 * P.C8;
-    P.neg_c4x4 = -4.0 * P.C4;
-    P.c8_a = P.c8x8 / P.m_a;
-    P.c4_a = P.neg_c4x4 / P.m_a;
-    P.c8_i = -P.c8x8 / P.m_i;
-    P.c4_i = -P.neg_c4x4 / P.m_i;
-    P.omega = tr->omega_rf_au;
-    P.T_rf = 2.0 * PI / P.omega;
-    for (int k = 0; k < 3; ++k) {
-        P.ka[k] = -tr->a[k] * (P.omega * P.omega / 4.0);
-        P.kq[k] = -2.0 * tr->q[k] * (P.omega * P.omega / 4.0);
-    }
-    c->w_harm = std::fabs(tr->q[0]) * P.omega / std::pow(2.0, 1.5);
-    P.rtol = T.rtol;
-    P.atol = T.atol;
-    P.thr = T.atol / T.rtol;
-    P.h_max = T.h_max_rf * P.T_rf;
-    P.h_min = std::ldexp(P.T_rf, -40);
-    P.t_max_rf = T.t_max_rf;
-    P.t_max = T.t_max_rf * P.T_rf;
-    P.h0_scale = 0.8 * std::pow(T.rtol, 0.2);
-    P.r0 = r0_a0;
-    P.r0sq = r0_a0 * r0_a0;
-    P.r_coll = T.r_coll_a0;
-    P.rcsq = T.r_coll_a0 * T.r_coll_a0;
-    P.loc_tol = 1e-13 * P.r0sq;
-    P.max_steps = T.max_steps;
-    P.n_near = T.t_max_rf > 2.0 ? (unsigned)std::floor(std::fmin(T.t_max_rf - 2.0, 4294967295.0)) : 0u;
-    const double d[16] = {P.m_i, P.m_a, P.C4, P.C8, P.De, P.r_e, P.omega, P.T_rf,
-                          P.thr, P.h_max, P.h_min, P.t_max, P.r0, P.r_coll, P.rtol, P.atol};
-    std::memcpy(c->derived, d, sizeof(d));
-    return IA_OK;
-}
-
 extern "C" int ia_run_static(const ia_species *species, const ia_trap *trap, double De_K, double r0_a0,
                              const ia_tol *tol, int cuda_device, const ia_launch *launch, const ia_outputs *outputs,
                              void *cuda_stream, char *errbuf, size_t errbuf_len) {
@@ -1059,7 +1006,7 @@ extern "C" int ia_run_static(const ia_species *species, const ia_trap *trap, dou
     if (launch->path != IA_PATH_AUTO)
         return static_fail(errbuf, errbuf_len, IA_EINVAL, "ia_run_static: launch.path must be IA_PATH_AUTO (it runs the production pair)");
     ia_ctx cell; /* host-only: parameters and error text; owns no stream, event or device memory */
-    int rc = prepare_cell(&cell, species, trap, De_K, r0_a0, tol);
+    int rc = prepare_cell(&cell.P, cell.derived, &cell.w_harm, species, trap, De_K, r0_a0, tol);
     if (rc != IA_OK)
         return static_fail(errbuf, errbuf_len, rc, "ia_run_static: a species, trap, well-depth, r0 or tolerance value is out of range");
     IaGen Gn;
